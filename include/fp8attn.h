@@ -1,0 +1,150 @@
+/*
+ * fp8attn.h -- C ABI of libfp8attn.so: B200 (sm_100a) FP8 attention forward with the
+ * kernel-faithful P-cast semantics of arxiv/paper_2606_06521.
+ *
+ * The operation is Algorithm 1 of the paper ("FP8 Online Softmax
+ * Attention") with the semantics of its section 6.1:
+ *     for each KV block j in BlockOrder:   Z = Q K_j^T / sqrt(d);  m_new = max(m, max Z);
+ *         alpha = exp(m - m_new);  P = exp(Z - m_new)  (FP32);
+ *         l = alpha l + sum(P)                      (FP32, PRE-cast P);
+ *         P8 = cast_E4M3(P * S)                     (round-to-nearest-even, saturating);
+ *         O = alpha O + P8 V_j                      (FP32 accumulate)
+ *     return O / (S l)
+ * BlockOrder is forward (0..nb-1) or reverse (nb-1..0, the block holding the sink keys
+ * last).  S is the static P scale (Eq. 16).
+ *
+ * All entry points return 0 on success or a negative FP8ATTN_E_* code; they never throw,
+ * abort or exit.  No entry point allocates or frees caller-visible memory or synchronises
+ * the stream.  Work is enqueued on the CUDA stream given in `stats->stream` (the legacy
+ * default stream if `stats` is NULL).  Scratch memory (split-KV partials, BF16 planes of
+ * FP32 inputs, quantised q for decode) is owned and cached by the library.
+ */
+#ifndef FP8ATTN_H
+#define FP8ATTN_H
+
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define FP8ATTN_API __attribute__((visibility("default")))
+
+/* ---- `mode` argument: (input dtype << 8) | P mode ------------------------------------ */
+#define FP8ATTN_MODE_NOCAST     0   /* reference: P stays FP32, S ignored (treated as 1)        */
+#define FP8ATTN_MODE_ISOLATION  1   /* P-cast isolation: Q,K,V FP32/BF16, P cast
+                                       to E4M3 and dequantised exactly to BF16 for P.V          */
+#define FP8ATTN_MODE_FP8        2   /* production: E4M3 q/k/v with per-(b,h) scales, both
+                                       matmuls tcgen05 kind::f8f6f4                            */
+#define FP8ATTN_DTYPE_F32          (0 << 8)  /* q,k,v float32                                    */
+#define FP8ATTN_DTYPE_BF16         (1 << 8)  /* q,k,v bfloat16                                   */
+#define FP8ATTN_DTYPE_E4M3         (2 << 8)  /* q,k,v E4M3 codes; q_scale,k_scale,v_scale needed */
+#define FP8ATTN_DTYPE_BF16Q_E4M3KV (3 << 8)  /* decode: q bfloat16 (quantised per (b,hq) slab to
+                                                E4M3 by the library), k,v E4M3; k_scale,v_scale  */
+
+/* ---- `kv_order` ---------------------------------------------------------------------- */
+#define FP8ATTN_ORDER_FORWARD 0     /* blocks 0 .. nb-1                                          */
+#define FP8ATTN_ORDER_REVERSE 1     /* blocks nb-1 .. 0 (sink block last)          */
+
+/* ---- error codes --------------------------------------------------------------------- */
+#define FP8ATTN_OK              0
+#define FP8ATTN_E_NULL         -1   /* a required pointer is NULL                                */
+#define FP8ATTN_E_SHAPE        -2   /* a size is < 1, Hq % Hkv != 0, or d not in {64, 128}       */
+#define FP8ATTN_E_SCALE        -3   /* S is not a finite FP32 > 0                                */
+#define FP8ATTN_E_MODE         -4   /* unknown mode / dtype / kv_order, or a combination that is
+                                       not defined (mode 2 needs E4M3 k,v; modes 0,1 need
+                                       FP32/BF16)                                               */
+#define FP8ATTN_E_UNSUPPORTED  -5   /* valid but not built: E4M3 with d != 128, block_n not in
+                                       {0, 64, 128}, FP32 inputs with block_n 128, num_splits
+                                       above FP8ATTN_MAX_SPLITS                                  */
+#define FP8ATTN_E_DEVICE       -6   /* current device is not compute capability 10.x             */
+#define FP8ATTN_E_CUDA         -7   /* a CUDA call failed (allocation, tensor map, launch)       */
+#define FP8ATTN_E_STATS        -8   /* stats->struct_size does not match this header             */
+
+#define FP8ATTN_MAX_SPLITS 64
+
+/*
+ * Optional controls and statistics.  Zero-initialise, set struct_size = sizeof(fp8attn_stats),
+ * fill what is needed.  Device pointers are caller-owned.
+ */
+typedef struct fp8attn_stats {
+    /* ---- inputs ---- */
+    int32_t struct_size;       /* sizeof(fp8attn_stats)                                          */
+    int32_t n_sink;            /* number of sink keys at the start of the sequence (k_sink,
+                                  PAPER.md:131); only used to classify underflows               */
+    int32_t block_n;           /* KV block size Bn request: 0 = library default, else 64 or 128
+                                  ("typically 64 or 128")                          */
+    int32_t num_splits;        /* split-KV request: 0 = automatic, n >= 1 = exactly n contiguous
+                                  block ranges                             */
+    const float *q_scale;      /* device [B*Hq]  dequantisation scale of E4M3 q (value = code*scale) */
+    const float *k_scale;      /* device [B*Hkv]                                                 */
+    const float *v_scale;      /* device [B*Hkv]                                                 */
+    void *stream;              /* cudaStream_t                                                   */
+    uint8_t *p_codes;          /* device [Lq, Lk] or NULL: E4M3 code of every P of head
+                                  (p_batch, p_head); masked positions hold 0xFF; mode 0 writes
+                                  nothing                                                       */
+    int32_t p_batch, p_head;
+    /* ---- outputs, device (each may be NULL) ---- */
+    float *row_max;            /* [B,Hq,Lq] final running max m (scaled logits, natural log)    */
+    float *row_sum;            /* [B,Hq,Lq] final l relative to m; NOT multiplied by S           */
+    unsigned long long *underflow; /* [2]: number of visible non-sink P values (key index >=
+                                  n_sink) whose E4M3 code is zero (Prop. 1),
+                                  [0] in blocks that hold a sink key, [1] in all other blocks.
+                                  Zeroed by the library at the start of the call.              */
+    /* ---- outputs, host (written before the call returns) ---- */
+    int32_t block_m_used;      /* query rows per tile                                            */
+    int32_t block_n_used;      /* Bn actually used                                               */
+    int32_t num_splits_used;
+    int32_t split_bounds[FP8ATTN_MAX_SPLITS + 1]; /* split s covers blocks
+                                  [split_bounds[s], split_bounds[s+1])                          */
+    int32_t kernel_id;         /* which kernel family ran: 1 = general tcgen05 kernel,
+                                  2 = warp-specialised prefill kernel, 3 = split-KV decode kernel */
+    int32_t n_launches;        /* kernels launched by this call                                  */
+} fp8attn_stats;
+
+/*
+ * fp8attn_fwd -- attention forward (Alg. 1).
+ *   q, o : device, [B, Hq, Lq, d] contiguous row-major; o is always float32.
+ *   k, v : device, [B, Hkv, Lk, d]; query head h reads kv head h / (Hq / Hkv).
+ *   d    : 64 or 128.  Softmax scale is 1/sqrt(d).
+ *   causal : nonzero = key j visible to query i iff j <= i + (Lk - Lq) (bottom-right).
+ *   S    : static P scale, finite > 0 (values above 448 saturate at 448).
+ *   kv_order, mode : see the defines above.
+ *   stats : NULL, or controls/statistics as documented in the struct.
+ * Rows that see no key produce 0, row_max = -inf, row_sum = 0.
+ */
+FP8ATTN_API int fp8attn_fwd(const void *q, const void *k, const void *v, void *o,
+                            int B, int Hq, int Hkv, int Lq, int Lk, int d,
+                            int causal, float S, int kv_order, int mode, fp8attn_stats *stats);
+
+/*
+ * fp8attn_quantize_e4m3 -- per-(b,h) slab quantisation of FP32 to E4M3 (BASELINE config 3
+ * "per-head absmax/448"; the paper treats QKV quantisation as orthogonal).
+ *   x : device float32 [B,H,L,d];  out_codes : device uint8 [B,H,L,d];
+ *   out_scale : device float32 [B,H] = absmax/448 (1 for an all-zero slab);
+ *   code = cvt.rn.satfinite.e4m3(x * (448/absmax)).  stream : cudaStream_t.
+ */
+FP8ATTN_API int fp8attn_quantize_e4m3(const float *x, uint8_t *out_codes, float *out_scale,
+                                      int B, int H, int L, int d, void *stream);
+
+/*
+ * fp8attn_debug_gemm -- one-tile tcgen05 GEMM through the same TMA / descriptor / TMEM
+ * helpers the attention kernels use; exists so tests can pin those primitives.
+ *   D[128,N] (device float32) = A[128,K] . B, FP32 accumulate.
+ *   elem_bytes 2 = BF16 (kind::f16), 1 = E4M3 (kind::f8f6f4).
+ *   a_in_tmem : 0 = A read from swizzled shared memory, 1 = A staged in TMEM (the P operand path).
+ *   b_mn_major: 0 = B given as [N,K] (K contiguous, the K-tile path), 1 = B given as [K,N]
+ *               (N contiguous, the V-tile path).
+ *   N in {64,128}; K a multiple of 64 (BF16) / 128 (E4M3), K <= 256.
+ */
+FP8ATTN_API int fp8attn_debug_gemm(const void *A, const void *Bm, float *D, int N, int K,
+                                   int elem_bytes, int a_in_tmem, int b_mn_major, void *stream);
+
+FP8ATTN_API const char *fp8attn_strerror(int code);
+FP8ATTN_API const char *fp8attn_last_cuda_error(void);   /* text of the last CUDA failure */
+FP8ATTN_API int fp8attn_version(void);                   /* major*10000 + minor*100 + patch */
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* FP8ATTN_H */

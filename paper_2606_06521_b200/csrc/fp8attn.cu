@@ -1,0 +1,397 @@
+// fp8attn.cu -- the C ABI of libfp8attn.so (include/fp8attn.h): argument checks, tensor maps,
+// library-owned scratch memory, kernel selection and launch.  No step of the method runs on
+// the host and there is no CPU fallback: without a compute-capability-10 device every entry
+// point that computes returns FP8ATTN_E_DEVICE.
+#include <cmath>
+#include <cstdarg>
+#include <cstring>
+#include <mutex>
+
+#include "../../include/fp8attn.h"
+#include "attn_general.cuh"
+#include "debug_gemm.cuh"
+#include "prep.cuh"
+
+namespace {
+
+using namespace fp8attn;
+
+thread_local char g_err[512] = "";
+
+void set_err(const char* fmt, ...) {
+    va_list ap;
+    va_start(ap, fmt);
+    vsnprintf(g_err, sizeof g_err, fmt, ap);
+    va_end(ap);
+}
+
+#define CU_TRY(expr)                                                                              \
+    do {                                                                                          \
+        cudaError_t e__ = (expr);                                                                 \
+        if (e__ != cudaSuccess) {                                                                 \
+            set_err("%s failed: %s (%s:%d)", #expr, cudaGetErrorString(e__), __FILE__, __LINE__); \
+            return FP8ATTN_E_CUDA;                                                                \
+        }                                                                                         \
+    } while (0)
+
+// ---------------------------------------------------------------------------- device check
+int check_device() {
+    int dev = 0;
+    if (cudaGetDevice(&dev) != cudaSuccess) {
+        cudaGetLastError();
+        set_err("no CUDA device");
+        return FP8ATTN_E_DEVICE;
+    }
+    static std::mutex mu;
+    static int cached_dev = -1, cached_rc = 0;
+    std::lock_guard<std::mutex> lock(mu);
+    if (dev == cached_dev) return cached_rc;
+    int major = 0;
+    if (cudaDeviceGetAttribute(&major, cudaDevAttrComputeCapabilityMajor, dev) != cudaSuccess) {
+        cudaGetLastError();
+        set_err("cannot query the device");
+        return FP8ATTN_E_DEVICE;
+    }
+    cached_dev = dev;
+    cached_rc = (major == 10) ? FP8ATTN_OK : FP8ATTN_E_DEVICE;
+    if (cached_rc) set_err("device %d has compute capability %d.x; sm_100 is required", dev, major);
+    return cached_rc;
+}
+
+// ---------------------------------------------------------------------------- tensor maps
+typedef CUresult (*EncodeTiledFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*,
+                                  const cuuint64_t*, const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave,
+                                  CUtensorMapSwizzle, CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+
+EncodeTiledFn encode_fn() {
+    static EncodeTiledFn fn = [] {
+        void* p = nullptr;
+        cudaDriverEntryPointQueryResult q;
+        if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &p, cudaEnableDefault, &q) != cudaSuccess) p = nullptr;
+        return reinterpret_cast<EncodeTiledFn>(p);
+    }();
+    return fn;
+}
+
+// [slabs, rows, cols] row-major, element size eb; box = one 128-byte chunk of `box_rows` rows, 128-byte swizzle.
+// Rows past `rows` read as zero.
+int make_map(CUtensorMap* m, const void* base, int eb, long long slabs, long long rows, int cols, int box_rows) {
+    EncodeTiledFn fn = encode_fn();
+    if (!fn) {
+        set_err("cuTensorMapEncodeTiled not available from the driver");
+        return FP8ATTN_E_CUDA;
+    }
+    const cuuint64_t gdim[3] = {(cuuint64_t)cols, (cuuint64_t)rows, (cuuint64_t)slabs};
+    const cuuint64_t gstr[2] = {(cuuint64_t)cols * eb, (cuuint64_t)cols * eb * (cuuint64_t)rows};
+    const cuuint32_t box[3] = {(cuuint32_t)(128 / eb), (cuuint32_t)box_rows, 1};
+    const cuuint32_t estr[3] = {1, 1, 1};
+    const CUtensorMapDataType dt = (eb == 2) ? CU_TENSOR_MAP_DATA_TYPE_BFLOAT16 : CU_TENSOR_MAP_DATA_TYPE_UINT8;
+    CUresult r = fn(m, dt, 3, const_cast<void*>(base), gdim, gstr, box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE,
+                    CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+    if (r != CUDA_SUCCESS) {
+        set_err("cuTensorMapEncodeTiled failed with CUresult %d (base %p eb %d slabs %lld rows %lld cols %d box %d)",
+                (int)r, base, eb, slabs, rows, cols, box_rows);
+        return FP8ATTN_E_CUDA;
+    }
+    return FP8ATTN_OK;
+}
+
+// ---------------------------------------------------------------------------- scratch memory
+// One growing stream-ordered buffer per purpose.  Freed and reallocated on the caller's stream,
+// so no host synchronisation is needed; kernels already enqueued keep their memory until they ran.
+struct Scratch {
+    void* ptr = nullptr;
+    size_t bytes = 0;
+    int dev = -1;
+    int get(void** out, size_t need, cudaStream_t st) {
+        int dev_now = 0;
+        cudaGetDevice(&dev_now);
+        if (ptr && (dev_now != dev || need > bytes)) {
+            cudaFreeAsync(ptr, st);
+            ptr = nullptr;
+            bytes = 0;
+        }
+        if (!ptr) {
+            size_t sz = need < 256 ? 256 : need;
+            CU_TRY(cudaMallocAsync(&ptr, sz, st));
+            bytes = sz;
+            dev = dev_now;
+        }
+        *out = ptr;
+        return FP8ATTN_OK;
+    }
+};
+std::mutex g_mu;                      // serialises calls that use the scratch buffers
+Scratch g_planes, g_partial, g_qquant, g_amax;
+
+// ---------------------------------------------------------------------------- general kernel launch
+template <int D, int BN, int EB, int NPL, int MODE>
+int launch_general(const CUtensorMap& mq, const CUtensorMap& mk, const CUtensorMap& mv, const FwdParams& p,
+                   dim3 grid, cudaStream_t st) {
+    using C = GeneralCfg<D, BN, EB, NPL, MODE>;
+    auto kern = attn_general_kernel<D, BN, EB, NPL, MODE>;
+    static bool configured = false;
+    if (!configured) {
+        CU_TRY(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, C::SMEM_BYTES));
+        configured = true;
+    }
+    kern<<<grid, 128, C::SMEM_BYTES, st>>>(mq, mk, mv, p);
+    CU_TRY(cudaGetLastError());
+    return FP8ATTN_OK;
+}
+
+template <int EB, int NPL, int MODE>
+int dispatch_general(int d, int bn, const CUtensorMap& mq, const CUtensorMap& mk, const CUtensorMap& mv,
+                     const FwdParams& p, dim3 grid, cudaStream_t st) {
+    if constexpr (NPL == 3) {   // FP32 inputs: Bn = 64 only (three planes of Q, K, V must fit in shared memory)
+        if (d == 64 && bn == 64) return launch_general<64, 64, EB, NPL, MODE>(mq, mk, mv, p, grid, st);
+        if (d == 128 && bn == 64) return launch_general<128, 64, EB, NPL, MODE>(mq, mk, mv, p, grid, st);
+    } else if constexpr (EB == 1) {   // E4M3: d = 128 only
+        if (d == 128 && bn == 64) return launch_general<128, 64, EB, NPL, MODE>(mq, mk, mv, p, grid, st);
+        if (d == 128 && bn == 128) return launch_general<128, 128, EB, NPL, MODE>(mq, mk, mv, p, grid, st);
+    } else {
+        if (d == 64 && bn == 64) return launch_general<64, 64, EB, NPL, MODE>(mq, mk, mv, p, grid, st);
+        if (d == 64 && bn == 128) return launch_general<64, 128, EB, NPL, MODE>(mq, mk, mv, p, grid, st);
+        if (d == 128 && bn == 64) return launch_general<128, 64, EB, NPL, MODE>(mq, mk, mv, p, grid, st);
+        if (d == 128 && bn == 128) return launch_general<128, 128, EB, NPL, MODE>(mq, mk, mv, p, grid, st);
+    }
+    set_err("no kernel instance for d=%d block_n=%d", d, bn);
+    return FP8ATTN_E_UNSUPPORTED;
+}
+
+}  // namespace
+
+// =============================================================================================
+// C ABI
+// =============================================================================================
+extern "C" {
+
+int fp8attn_version(void) { return 100; }   // 0.1.0
+
+const char* fp8attn_last_cuda_error(void) { return g_err; }
+
+const char* fp8attn_strerror(int code) {
+    switch (code) {
+        case FP8ATTN_OK: return "success";
+        case FP8ATTN_E_NULL: return "a required pointer is NULL";
+        case FP8ATTN_E_SHAPE: return "bad shape: sizes must be >= 1, Hq % Hkv == 0, d in {64, 128}";
+        case FP8ATTN_E_SCALE: return "S must be a finite float > 0";
+        case FP8ATTN_E_MODE: return "unknown or inconsistent mode / dtype / kv_order";
+        case FP8ATTN_E_UNSUPPORTED: return "valid request that this build does not support";
+        case FP8ATTN_E_DEVICE: return "the current device is not compute capability 10.x";
+        case FP8ATTN_E_CUDA: return "a CUDA call failed (see fp8attn_last_cuda_error)";
+        case FP8ATTN_E_STATS: return "stats->struct_size does not match this header";
+        default: return "unknown error code";
+    }
+}
+
+int fp8attn_fwd(const void* q, const void* k, const void* v, void* o, int B, int Hq, int Hkv, int Lq, int Lk, int d,
+                int causal, float S, int kv_order, int mode, fp8attn_stats* stats) {
+    // ---- argument checks: no CUDA call before these pass ----
+    if (!q || !k || !v || !o) return FP8ATTN_E_NULL;
+    if (B < 1 || Hq < 1 || Hkv < 1 || Lq < 1 || Lk < 1) return FP8ATTN_E_SHAPE;
+    if (Hq % Hkv != 0 || (d != 64 && d != 128)) return FP8ATTN_E_SHAPE;
+    if (!(S > 0.0f) || !std::isfinite(S)) return FP8ATTN_E_SCALE;
+    const int pm = mode & 0xFF, dt = (mode >> 8) & 0xF;
+    if ((mode & ~0xFFF) || pm > 2 || dt > 3) return FP8ATTN_E_MODE;
+    if (kv_order != FP8ATTN_ORDER_FORWARD && kv_order != FP8ATTN_ORDER_REVERSE) return FP8ATTN_E_MODE;
+    const bool e4m3_kv = (dt == 2 || dt == 3);
+    if ((pm == FP8ATTN_MODE_FP8) != e4m3_kv) return FP8ATTN_E_MODE;
+    if (stats && stats->struct_size != (int32_t)sizeof(fp8attn_stats)) return FP8ATTN_E_STATS;
+    if (e4m3_kv) {
+        if (!stats || !stats->k_scale || !stats->v_scale) return FP8ATTN_E_NULL;
+        if (dt == 2 && !stats->q_scale) return FP8ATTN_E_NULL;
+        if (d != 128) return FP8ATTN_E_UNSUPPORTED;
+    }
+    int bn = stats ? stats->block_n : 0;
+    if (bn != 0 && bn != 64 && bn != 128) return FP8ATTN_E_UNSUPPORTED;
+    if (dt == 0 && bn == 128) return FP8ATTN_E_UNSUPPORTED;
+    if (bn == 0) bn = (dt == 0) ? 64 : 128;
+    int ns = stats ? stats->num_splits : 0;
+    if (ns < 0 || ns > FP8ATTN_MAX_SPLITS) return FP8ATTN_E_UNSUPPORTED;
+    if (stats && stats->p_codes && (stats->p_batch < 0 || stats->p_batch >= B || stats->p_head < 0 || stats->p_head >= Hq))
+        return FP8ATTN_E_SHAPE;
+    const long long q_slabs = (long long)B * Hq, kv_slabs = (long long)B * Hkv;
+    if (q_slabs > 65535) return FP8ATTN_E_UNSUPPORTED;
+    if (int rc = check_device()) return rc;
+
+    cudaStream_t st = stats ? reinterpret_cast<cudaStream_t>(stats->stream) : nullptr;
+    const int nb = (Lk + bn - 1) / bn;
+    const int n_qtiles = (Lq + BM - 1) / BM;
+    if (ns == 0) {
+        // automatic: split only decode-shaped calls (a handful of query rows per head) whose query
+        // tiles alone cannot fill the GPU.  Splitting changes which P values are cast against the
+        // sink's running max (reading R14), so prefill is never split behind the caller's back.
+        const long long tiles = (long long)n_qtiles * q_slabs;
+        ns = 1;
+        if (Lq <= 16 && tiles < 2 * 148 && nb > 1) {
+            long long want = (4 * 148 + tiles - 1) / tiles;
+            ns = (int)(want < nb ? want : nb);
+            if (ns > FP8ATTN_MAX_SPLITS) ns = FP8ATTN_MAX_SPLITS;
+        }
+    }
+    if (ns > nb) ns = nb;
+
+    std::lock_guard<std::mutex> lock(g_mu);
+    const long long nq = q_slabs * Lq * d, nkv = kv_slabs * Lk * d;
+    const void *qs = q, *ks = k, *vs = v;   // staged operands the kernel reads
+    const float* q_scale = stats ? stats->q_scale : nullptr;
+    int n_launches = 0;
+    int eb = 2, npl = 1;
+    if (dt == 0) {
+        // FP32 -> three BF16 planes each (exact split), so that tcgen05 reproduces FP32 logits
+        void* ws = nullptr;
+        if (int rc = g_planes.get(&ws, (size_t)(nq + 2 * nkv) * 3 * 2, st)) return rc;
+        uint16_t* pq = static_cast<uint16_t*>(ws);
+        uint16_t* pk = pq + 3 * nq;
+        uint16_t* pv = pk + 3 * nkv;
+        const int thr = 256;
+        auto blocks = [&](long long n) { long long b = (n / 4 + thr - 1) / thr; return (unsigned)(b < 1 ? 1 : (b > 148 * 16 ? 148 * 16 : b)); };
+        split_planes_kernel<<<blocks(nq), thr, 0, st>>>(static_cast<const float*>(q), pq, nq);
+        split_planes_kernel<<<blocks(nkv), thr, 0, st>>>(static_cast<const float*>(k), pk, nkv);
+        split_planes_kernel<<<blocks(nkv), thr, 0, st>>>(static_cast<const float*>(v), pv, nkv);
+        CU_TRY(cudaGetLastError());
+        n_launches += 3;
+        qs = pq; ks = pk; vs = pv;
+        npl = 3;
+    } else if (dt == 2) {
+        eb = 1;
+    } else if (dt == 3) {
+        // decode: quantise the BF16 q of every (b, hq) slab to E4M3 (reading R8 in DESIGN.md)
+        eb = 1;
+        void *wq = nullptr, *wa = nullptr;
+        if (int rc = g_qquant.get(&wq, (size_t)nq + (size_t)q_slabs * 4 + 16, st)) return rc;
+        if (int rc = g_amax.get(&wa, (size_t)q_slabs * 4, st)) return rc;
+        uint8_t* codes = static_cast<uint8_t*>(wq);
+        float* qsc = reinterpret_cast<float*>(codes + ((nq + 15) / 16) * 16);
+        unsigned int* amax = static_cast<unsigned int*>(wa);
+        const long long slab = (long long)Lq * d;
+        CU_TRY(cudaMemsetAsync(amax, 0, (size_t)q_slabs * 4, st));
+        unsigned gx = (unsigned)((slab + 255) / 256);
+        if (gx > 64) gx = 64;
+        absmax_kernel<__nv_bfloat16><<<dim3(gx, (unsigned)q_slabs), 256, 0, st>>>(static_cast<const __nv_bfloat16*>(q), amax, slab);
+        quantize_kernel<__nv_bfloat16><<<dim3(gx, (unsigned)q_slabs), 256, 0, st>>>(static_cast<const __nv_bfloat16*>(q), amax, codes, slab);
+        finalize_scale_kernel<<<(unsigned)((q_slabs + 255) / 256), 256, 0, st>>>(amax, qsc, (int)q_slabs);
+        CU_TRY(cudaGetLastError());
+        n_launches += 3;
+        qs = codes;
+        q_scale = qsc;
+    }
+
+    CUtensorMap mq, mk, mv;
+    if (int rc = make_map(&mq, qs, eb, npl * q_slabs, Lq, d, BM)) return rc;
+    if (int rc = make_map(&mk, ks, eb, npl * kv_slabs, Lk, d, bn)) return rc;
+    if (int rc = make_map(&mv, vs, eb, npl * kv_slabs, Lk, d, bn)) return rc;
+
+    FwdParams p;
+    memset(&p, 0, sizeof p);
+    p.o = static_cast<float*>(o);
+    p.row_max = stats ? stats->row_max : nullptr;
+    p.row_sum = stats ? stats->row_sum : nullptr;
+    p.underflow = stats ? stats->underflow : nullptr;
+    p.p_codes = stats ? stats->p_codes : nullptr;
+    p.p_bh = stats ? stats->p_batch * Hq + stats->p_head : 0;
+    p.q_scale = q_scale;
+    p.k_scale = stats ? stats->k_scale : nullptr;
+    p.v_scale = stats ? stats->v_scale : nullptr;
+    p.B = B; p.Hq = Hq; p.Hkv = Hkv; p.Lq = Lq; p.Lk = Lk;
+    p.causal = causal ? 1 : 0;
+    p.kv_order = kv_order;
+    p.n_sink = stats ? stats->n_sink : 0;
+    p.num_splits = ns;
+    p.nb = nb;
+    p.q_slabs = (int)q_slabs;
+    p.kv_slabs = (int)kv_slabs;
+    p.S = S;
+    p.sm_scale = 1.0f / sqrtf((float)d);
+    const long long R = q_slabs * Lq;
+    if (ns > 1) {
+        void* ws = nullptr;
+        if (int rc = g_partial.get(&ws, (size_t)ns * R * (d + 2) * 4, st)) return rc;
+        p.part_o = static_cast<float*>(ws);
+        p.part_ml = p.part_o + (size_t)ns * R * d;
+    }
+    if (p.underflow) CU_TRY(cudaMemsetAsync(p.underflow, 0, 2 * sizeof(unsigned long long), st));
+
+    const dim3 grid((unsigned)n_qtiles, (unsigned)q_slabs, (unsigned)ns);
+    int rc;
+    if (npl == 3)
+        rc = (pm == 0) ? dispatch_general<2, 3, 0>(d, bn, mq, mk, mv, p, grid, st)
+                       : dispatch_general<2, 3, 1>(d, bn, mq, mk, mv, p, grid, st);
+    else if (eb == 2)
+        rc = (pm == 0) ? dispatch_general<2, 1, 0>(d, bn, mq, mk, mv, p, grid, st)
+                       : dispatch_general<2, 1, 1>(d, bn, mq, mk, mv, p, grid, st);
+    else
+        rc = dispatch_general<1, 1, 2>(d, bn, mq, mk, mv, p, grid, st);
+    if (rc) return rc;
+    ++n_launches;
+    if (ns > 1) {
+        const int rows_per_block = 8;
+        combine_kernel<<<(unsigned)((R + rows_per_block - 1) / rows_per_block), rows_per_block * 32, 0, st>>>(
+            p.part_o, p.part_ml, p.o, p.row_max, p.row_sum, (pm == 2) ? p.v_scale : nullptr, R, d, ns,
+            (pm == 0) ? 1.0f : S, Hq, Hkv, Lq);
+        CU_TRY(cudaGetLastError());
+        ++n_launches;
+    }
+    if (stats) {
+        stats->block_m_used = BM;
+        stats->block_n_used = bn;
+        stats->num_splits_used = ns;
+        for (int s = 0; s <= ns; ++s) stats->split_bounds[s] = (int)(((long long)s * nb) / ns);
+        stats->kernel_id = 1;
+        stats->n_launches = n_launches;
+    }
+    return FP8ATTN_OK;
+}
+
+int fp8attn_quantize_e4m3(const float* x, uint8_t* out_codes, float* out_scale, int B, int H, int L, int d,
+                          void* stream) {
+    if (!x || !out_codes || !out_scale) return FP8ATTN_E_NULL;
+    if (B < 1 || H < 1 || L < 1 || d < 1) return FP8ATTN_E_SHAPE;
+    if (int rc = check_device()) return rc;
+    cudaStream_t st = reinterpret_cast<cudaStream_t>(stream);
+    const long long slabs = (long long)B * H, slab = (long long)L * d;
+    if (slabs > 65535) return FP8ATTN_E_UNSUPPORTED;
+    std::lock_guard<std::mutex> lock(g_mu);
+    void* wa = nullptr;
+    if (int rc = g_amax.get(&wa, (size_t)slabs * 4, st)) return rc;
+    unsigned int* amax = static_cast<unsigned int*>(wa);
+    CU_TRY(cudaMemsetAsync(amax, 0, (size_t)slabs * 4, st));
+    unsigned gx = (unsigned)((slab + 1023) / 1024);
+    if (gx > 148) gx = 148;
+    absmax_kernel<float><<<dim3(gx, (unsigned)slabs), 256, 0, st>>>(x, amax, slab);
+    quantize_kernel<float><<<dim3(gx, (unsigned)slabs), 256, 0, st>>>(x, amax, out_codes, slab);
+    finalize_scale_kernel<<<(unsigned)((slabs + 255) / 256), 256, 0, st>>>(amax, out_scale, (int)slabs);
+    CU_TRY(cudaGetLastError());
+    return FP8ATTN_OK;
+}
+
+int fp8attn_debug_gemm(const void* A, const void* Bm, float* D, int N, int K, int elem_bytes, int a_in_tmem,
+                       int b_mn_major, void* stream) {
+    if (!A || !Bm || !D) return FP8ATTN_E_NULL;
+    if ((elem_bytes != 1 && elem_bytes != 2) || (N != 64 && N != 128)) return FP8ATTN_E_SHAPE;
+    const int ch = 128 / elem_bytes;
+    if (K < ch || K % ch != 0 || K > 256) return FP8ATTN_E_SHAPE;
+    if (int rc = check_device()) return rc;
+    cudaStream_t st = reinterpret_cast<cudaStream_t>(stream);
+    CUtensorMap ma, mb;
+    if (int rc = make_map(&ma, A, elem_bytes, 1, 128, K, 128)) return rc;
+    if (b_mn_major) {
+        if (int rc = make_map(&mb, Bm, elem_bytes, 1, K, N, K)) return rc;     // [K, N]: boxes of K rows x 128 B
+    } else {
+        if (int rc = make_map(&mb, Bm, elem_bytes, 1, N, K, N)) return rc;     // [N, K]: boxes of N rows x 128 B
+    }
+    const int smem = (K / ch) * 128 * 128 + (b_mn_major ? (N / ch > 0 ? N / ch : 1) * K * 128 : (K / ch) * N * 128) + 1024 + 64;
+    if (b_mn_major && N < ch) return FP8ATTN_E_SHAPE;
+    if (elem_bytes == 2) {
+        CU_TRY(cudaFuncSetAttribute(debug_gemm_kernel<2>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
+        debug_gemm_kernel<2><<<1, 128, smem, st>>>(ma, mb, static_cast<const uint8_t*>(A), D, N, K, a_in_tmem, b_mn_major);
+    } else {
+        CU_TRY(cudaFuncSetAttribute(debug_gemm_kernel<1>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
+        debug_gemm_kernel<1><<<1, 128, smem, st>>>(ma, mb, static_cast<const uint8_t*>(A), D, N, K, a_in_tmem, b_mn_major);
+    }
+    CU_TRY(cudaGetLastError());
+    return FP8ATTN_OK;
+}
+
+}  // extern "C"
