@@ -118,6 +118,21 @@ FP8ATTN_API int fp8attn_fwd(const void *q, const void *k, const void *v, void *o
                             int causal, float S, int kv_order, int mode, fp8attn_stats *stats);
 
 /*
+ * fp8attn_fwd_host -- the same operation with HOST buffers (the end-to-end call).
+ *   q, k, v, o and, in `stats`, q_scale / k_scale / v_scale / row_max / row_sum / underflow /
+ *   p_codes are HOST pointers here (pinned memory makes the copies asynchronous; pageable
+ *   memory works).  The library copies q, k, v and the scales to library-owned device scratch
+ *   on `stats->stream`, runs fp8attn_fwd there, copies o and the requested statistics back and
+ *   synchronises that stream before returning, so the outputs are valid on return.
+ *   Element sizes follow the dtype bits of `mode`: FP32 4 B, BF16 2 B, E4M3 1 B.
+ * Every step of the method still runs in the CUDA kernels; the host side only copies.
+ * Errors as fp8attn_fwd.
+ */
+FP8ATTN_API int fp8attn_fwd_host(const void *q, const void *k, const void *v, void *o,
+                                 int B, int Hq, int Hkv, int Lq, int Lk, int d,
+                                 int causal, float S, int kv_order, int mode, fp8attn_stats *stats);
+
+/*
  * fp8attn_quantize_e4m3 -- per-(b,h) slab quantisation of FP32 to E4M3 (BASELINE config 3
  * "per-head absmax/448"; the paper treats QKV quantisation as orthogonal).
  *   x : device float32 [B,H,L,d];  out_codes : device uint8 [B,H,L,d];

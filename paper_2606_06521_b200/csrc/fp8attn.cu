@@ -159,6 +159,35 @@ int dispatch_general(int d, int bn, const CUtensorMap& mq, const CUtensorMap& mk
     return FP8ATTN_E_UNSUPPORTED;
 }
 
+// Argument checks shared by fp8attn_fwd and fp8attn_fwd_host: no CUDA call before these pass.
+int validate_args(const void* q, const void* k, const void* v, const void* o, int B, int Hq, int Hkv, int Lq, int Lk,
+                  int d, float S, int kv_order, int mode, const fp8attn_stats* stats) {
+    if (!q || !k || !v || !o) return FP8ATTN_E_NULL;
+    if (B < 1 || Hq < 1 || Hkv < 1 || Lq < 1 || Lk < 1) return FP8ATTN_E_SHAPE;
+    if (Hq % Hkv != 0 || (d != 64 && d != 128)) return FP8ATTN_E_SHAPE;
+    if (!(S > 0.0f) || !std::isfinite(S)) return FP8ATTN_E_SCALE;
+    const int pm = mode & 0xFF, dt = (mode >> 8) & 0xF;
+    if ((mode & ~0xFFF) || pm > 2 || dt > 3) return FP8ATTN_E_MODE;
+    if (kv_order != FP8ATTN_ORDER_FORWARD && kv_order != FP8ATTN_ORDER_REVERSE) return FP8ATTN_E_MODE;
+    const bool e4m3_kv = (dt == 2 || dt == 3);
+    if ((pm == FP8ATTN_MODE_FP8) != e4m3_kv) return FP8ATTN_E_MODE;
+    if (stats && stats->struct_size != (int32_t)sizeof(fp8attn_stats)) return FP8ATTN_E_STATS;
+    if (e4m3_kv) {
+        if (!stats || !stats->k_scale || !stats->v_scale) return FP8ATTN_E_NULL;
+        if (dt == 2 && !stats->q_scale) return FP8ATTN_E_NULL;
+        if (d != 128) return FP8ATTN_E_UNSUPPORTED;
+    }
+    const int bn = stats ? stats->block_n : 0;
+    if (bn != 0 && bn != 64 && bn != 128) return FP8ATTN_E_UNSUPPORTED;
+    if (dt == 0 && bn == 128) return FP8ATTN_E_UNSUPPORTED;
+    const int ns = stats ? stats->num_splits : 0;
+    if (ns < 0 || ns > FP8ATTN_MAX_SPLITS) return FP8ATTN_E_UNSUPPORTED;
+    if (stats && stats->p_codes && (stats->p_batch < 0 || stats->p_batch >= B || stats->p_head < 0 || stats->p_head >= Hq))
+        return FP8ATTN_E_SHAPE;
+    if ((long long)B * Hq > 65535) return FP8ATTN_E_UNSUPPORTED;
+    return FP8ATTN_OK;
+}
+
 }  // namespace
 
 // =============================================================================================
@@ -187,32 +216,12 @@ const char* fp8attn_strerror(int code) {
 
 int fp8attn_fwd(const void* q, const void* k, const void* v, void* o, int B, int Hq, int Hkv, int Lq, int Lk, int d,
                 int causal, float S, int kv_order, int mode, fp8attn_stats* stats) {
-    // ---- argument checks: no CUDA call before these pass ----
-    if (!q || !k || !v || !o) return FP8ATTN_E_NULL;
-    if (B < 1 || Hq < 1 || Hkv < 1 || Lq < 1 || Lk < 1) return FP8ATTN_E_SHAPE;
-    if (Hq % Hkv != 0 || (d != 64 && d != 128)) return FP8ATTN_E_SHAPE;
-    if (!(S > 0.0f) || !std::isfinite(S)) return FP8ATTN_E_SCALE;
+    if (int rc = validate_args(q, k, v, o, B, Hq, Hkv, Lq, Lk, d, S, kv_order, mode, stats)) return rc;
     const int pm = mode & 0xFF, dt = (mode >> 8) & 0xF;
-    if ((mode & ~0xFFF) || pm > 2 || dt > 3) return FP8ATTN_E_MODE;
-    if (kv_order != FP8ATTN_ORDER_FORWARD && kv_order != FP8ATTN_ORDER_REVERSE) return FP8ATTN_E_MODE;
-    const bool e4m3_kv = (dt == 2 || dt == 3);
-    if ((pm == FP8ATTN_MODE_FP8) != e4m3_kv) return FP8ATTN_E_MODE;
-    if (stats && stats->struct_size != (int32_t)sizeof(fp8attn_stats)) return FP8ATTN_E_STATS;
-    if (e4m3_kv) {
-        if (!stats || !stats->k_scale || !stats->v_scale) return FP8ATTN_E_NULL;
-        if (dt == 2 && !stats->q_scale) return FP8ATTN_E_NULL;
-        if (d != 128) return FP8ATTN_E_UNSUPPORTED;
-    }
     int bn = stats ? stats->block_n : 0;
-    if (bn != 0 && bn != 64 && bn != 128) return FP8ATTN_E_UNSUPPORTED;
-    if (dt == 0 && bn == 128) return FP8ATTN_E_UNSUPPORTED;
     if (bn == 0) bn = (dt == 0) ? 64 : 128;
     int ns = stats ? stats->num_splits : 0;
-    if (ns < 0 || ns > FP8ATTN_MAX_SPLITS) return FP8ATTN_E_UNSUPPORTED;
-    if (stats && stats->p_codes && (stats->p_batch < 0 || stats->p_batch >= B || stats->p_head < 0 || stats->p_head >= Hq))
-        return FP8ATTN_E_SHAPE;
     const long long q_slabs = (long long)B * Hq, kv_slabs = (long long)B * Hkv;
-    if (q_slabs > 65535) return FP8ATTN_E_UNSUPPORTED;
     if (int rc = check_device()) return rc;
 
     cudaStream_t st = stats ? reinterpret_cast<cudaStream_t>(stats->stream) : nullptr;
@@ -341,6 +350,88 @@ int fp8attn_fwd(const void* q, const void* k, const void* v, void* o, int B, int
         stats->kernel_id = 1;
         stats->n_launches = n_launches;
     }
+    return FP8ATTN_OK;
+}
+
+int fp8attn_fwd_host(const void* q, const void* k, const void* v, void* o, int B, int Hq, int Hkv, int Lq, int Lk,
+                     int d, int causal, float S, int kv_order, int mode, fp8attn_stats* stats) {
+    if (int rc = validate_args(q, k, v, o, B, Hq, Hkv, Lq, Lk, d, S, kv_order, mode, stats)) return rc;
+    if (int rc = check_device()) return rc;
+    const int dt = (mode >> 8) & 0xF;
+    const size_t ebq = (dt == 0) ? 4 : (dt == 2 ? 1 : 2);
+    const size_t ebkv = (dt == 0) ? 4 : (dt == 1 ? 2 : 1);
+    const size_t R = (size_t)B * Hq * Lq;
+    const size_t nq = R * d, nkv = (size_t)B * Hkv * Lk * d;
+    const size_t nqs = (size_t)B * Hq, nkvs = (size_t)B * Hkv;
+    auto up = [](size_t x) { return (x + 255) & ~size_t(255); };
+    // device staging layout
+    size_t off = 0;
+    const size_t o_q = off;   off += up(nq * ebq);
+    const size_t o_k = off;   off += up(nkv * ebkv);
+    const size_t o_v = off;   off += up(nkv * ebkv);
+    const size_t o_o = off;   off += up(nq * 4);
+    const size_t o_qs = off;  off += up(nqs * 4);
+    const size_t o_ks = off;  off += up(nkvs * 4);
+    const size_t o_vs = off;  off += up(nkvs * 4);
+    const size_t o_rm = off;  off += up(R * 4);
+    const size_t o_rs = off;  off += up(R * 4);
+    const size_t o_uf = off;  off += up(16);
+    const size_t o_pc = off;  off += (stats && stats->p_codes) ? up((size_t)Lq * Lk) : 0;
+
+    cudaStream_t st = stats ? reinterpret_cast<cudaStream_t>(stats->stream) : nullptr;
+    static std::mutex host_mu;
+    static Scratch host_buf;
+    std::lock_guard<std::mutex> lock(host_mu);
+    void* ws = nullptr;
+    if (int rc = host_buf.get(&ws, off, st)) return rc;
+    uint8_t* base = static_cast<uint8_t*>(ws);
+    CU_TRY(cudaMemcpyAsync(base + o_q, q, nq * ebq, cudaMemcpyHostToDevice, st));
+    CU_TRY(cudaMemcpyAsync(base + o_k, k, nkv * ebkv, cudaMemcpyHostToDevice, st));
+    CU_TRY(cudaMemcpyAsync(base + o_v, v, nkv * ebkv, cudaMemcpyHostToDevice, st));
+
+    fp8attn_stats dstats;
+    fp8attn_stats* ds = nullptr;
+    if (stats) {
+        dstats = *stats;
+        ds = &dstats;
+        if (stats->q_scale) {
+            CU_TRY(cudaMemcpyAsync(base + o_qs, stats->q_scale, nqs * 4, cudaMemcpyHostToDevice, st));
+            dstats.q_scale = reinterpret_cast<const float*>(base + o_qs);
+        }
+        if (stats->k_scale) {
+            CU_TRY(cudaMemcpyAsync(base + o_ks, stats->k_scale, nkvs * 4, cudaMemcpyHostToDevice, st));
+            dstats.k_scale = reinterpret_cast<const float*>(base + o_ks);
+        }
+        if (stats->v_scale) {
+            CU_TRY(cudaMemcpyAsync(base + o_vs, stats->v_scale, nkvs * 4, cudaMemcpyHostToDevice, st));
+            dstats.v_scale = reinterpret_cast<const float*>(base + o_vs);
+        }
+        if (stats->row_max) dstats.row_max = reinterpret_cast<float*>(base + o_rm);
+        if (stats->row_sum) dstats.row_sum = reinterpret_cast<float*>(base + o_rs);
+        if (stats->underflow) dstats.underflow = reinterpret_cast<unsigned long long*>(base + o_uf);
+        if (stats->p_codes) {
+            dstats.p_codes = base + o_pc;
+            CU_TRY(cudaMemsetAsync(base + o_pc, 0xFF, (size_t)Lq * Lk, st));
+        }
+    }
+    if (int rc = fp8attn_fwd(base + o_q, base + o_k, base + o_v, base + o_o, B, Hq, Hkv, Lq, Lk, d, causal, S,
+                             kv_order, mode, ds))
+        return rc;
+    CU_TRY(cudaMemcpyAsync(o, base + o_o, nq * 4, cudaMemcpyDeviceToHost, st));
+    if (stats) {
+        if (stats->row_max) CU_TRY(cudaMemcpyAsync(stats->row_max, base + o_rm, R * 4, cudaMemcpyDeviceToHost, st));
+        if (stats->row_sum) CU_TRY(cudaMemcpyAsync(stats->row_sum, base + o_rs, R * 4, cudaMemcpyDeviceToHost, st));
+        if (stats->underflow) CU_TRY(cudaMemcpyAsync(stats->underflow, base + o_uf, 16, cudaMemcpyDeviceToHost, st));
+        if (stats->p_codes)
+            CU_TRY(cudaMemcpyAsync(stats->p_codes, base + o_pc, (size_t)Lq * Lk, cudaMemcpyDeviceToHost, st));
+        stats->block_m_used = dstats.block_m_used;
+        stats->block_n_used = dstats.block_n_used;
+        stats->num_splits_used = dstats.num_splits_used;
+        memcpy(stats->split_bounds, dstats.split_bounds, sizeof dstats.split_bounds);
+        stats->kernel_id = dstats.kernel_id;
+        stats->n_launches = dstats.n_launches;
+    }
+    CU_TRY(cudaStreamSynchronize(st));
     return FP8ATTN_OK;
 }
 

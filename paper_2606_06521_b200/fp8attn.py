@@ -44,6 +44,8 @@ def _load():
     lib.fp8attn_fwd.argtypes = [C.c_void_p] * 4 + [C.c_int] * 7 + [C.c_float, C.c_int, C.c_int,
                                                                   C.POINTER(Stats)]
     lib.fp8attn_fwd.restype = C.c_int
+    lib.fp8attn_fwd_host.argtypes = lib.fp8attn_fwd.argtypes
+    lib.fp8attn_fwd_host.restype = C.c_int
     lib.fp8attn_quantize_e4m3.argtypes = [C.c_void_p] * 3 + [C.c_int] * 4 + [C.c_void_p]
     lib.fp8attn_quantize_e4m3.restype = C.c_int
     lib.fp8attn_debug_gemm.argtypes = [C.c_void_p] * 3 + [C.c_int] * 5 + [C.c_void_p]
@@ -59,6 +61,7 @@ _lib = _load()
 LIB_PATH = _lib._name
 
 fp8attn_fwd = _lib.fp8attn_fwd
+fp8attn_fwd_host = _lib.fp8attn_fwd_host
 fp8attn_quantize_e4m3 = _lib.fp8attn_quantize_e4m3
 fp8attn_debug_gemm = _lib.fp8attn_debug_gemm
 fp8attn_version = _lib.fp8attn_version
@@ -157,6 +160,45 @@ def fwd(q, k, v, *, causal: bool, S: float, kv_order: int, mode: int, n_sink: in
     _check(rc)
     ns = st.num_splits_used
     return FwdResult(o, row_max, row_sum, underflow, codes, st.block_m_used, st.block_n_used, ns,
+                     [st.split_bounds[i] for i in range(ns + 1)], st.kernel_id, st.n_launches)
+
+
+def fwd_host(q, k, v, *, causal: bool, S: float, kv_order: int, mode: int, n_sink: int = 4,
+             block_n: int = 0, num_splits: int = 0, q_scale=None, k_scale=None, v_scale=None,
+             want_stats: bool = False, out=None, stream=None, device=None) -> FwdResult:
+    """fp8attn_fwd_host on HOST tensors (CPU, ideally pinned): the library copies them to the
+    device, runs the kernels, copies `o` (and statistics) back and synchronises the stream."""
+    for t in (q, k, v):
+        if t.is_cuda or not t.is_contiguous() or t.dim() != 4:
+            raise ValueError("q, k, v must be contiguous 4-D CPU tensors")
+    B, Hq, Lq, d = q.shape
+    Bk, Hkv, Lk, dk = k.shape
+    if (Bk, dk) != (B, d) or v.shape != k.shape:
+        raise ValueError("shape mismatch between q, k, v")
+    o = out if out is not None else torch.empty((B, Hq, Lq, d), dtype=torch.float32, pin_memory=True)
+    st = Stats()
+    st.struct_size = C.sizeof(Stats)
+    st.n_sink, st.block_n, st.num_splits = n_sink, block_n, num_splits
+    keep = []
+    for name, t in (("q_scale", q_scale), ("k_scale", k_scale), ("v_scale", v_scale)):
+        if t is not None:
+            t = t.to(device="cpu", dtype=torch.float32).contiguous()
+            keep.append(t)
+            setattr(st, name, t.data_ptr())
+    row_max = row_sum = underflow = None
+    if want_stats:
+        row_max = torch.empty((B, Hq, Lq), dtype=torch.float32, pin_memory=True)
+        row_sum = torch.empty((B, Hq, Lq), dtype=torch.float32, pin_memory=True)
+        underflow = torch.zeros(2, dtype=torch.int64, pin_memory=True)
+        st.row_max, st.row_sum, st.underflow = row_max.data_ptr(), row_sum.data_ptr(), underflow.data_ptr()
+    dev = torch.device("cuda", torch.cuda.current_device()) if device is None else torch.device(device)
+    with torch.cuda.device(dev):
+        st.stream = _stream_ptr(stream)
+        rc = fp8attn_fwd_host(_ptr(q), _ptr(k), _ptr(v), _ptr(o), B, Hq, Hkv, Lq, Lk, d, int(bool(causal)),
+                              float(S), int(kv_order), int(mode) | _dtype_code(q, k), C.byref(st))
+    _check(rc)
+    ns = st.num_splits_used
+    return FwdResult(o, row_max, row_sum, underflow, None, st.block_m_used, st.block_n_used, ns,
                      [st.split_bounds[i] for i in range(ns + 1)], st.kernel_id, st.n_launches)
 
 

@@ -93,3 +93,18 @@ def sample_rows(B, Hq, Lq, n_per_head, seed=0, heads=None):
             idx = np.unique(idx)
         out.append(bh * Lq + idx)
     return np.concatenate(out).astype(np.int64)
+
+
+def batch_qkv(cfg: Config, b: int, seed=0, delta=None):
+    """Batch element `b` of a large config (cfg3..cfg5), drawn on its own from
+    default_rng([seed, b]) so that bench and tests can build the workload piece by piece:
+    Q [Hq,Lq,d], K, V [Hkv,Lk,d] (FP32, sink construction as in sink_qkv)."""
+    rng = np.random.default_rng([seed, b])
+    d = cfg.d
+    q = rng.standard_normal((cfg.Hq, cfg.Lq, d), dtype=np.float32)
+    k = rng.standard_normal((cfg.Hkv, cfg.Lk, d), dtype=np.float32)
+    v = rng.standard_normal((cfg.Hkv, cfg.Lk, d), dtype=np.float32)
+    q[..., d - 1] = 1.0
+    k[..., d - 1] = 0.0
+    k[..., :cfg.n_sink, d - 1] = np.float32((cfg.delta if delta is None else delta) * np.sqrt(d))
+    return q, k, v

@@ -1,0 +1,137 @@
+"""Shared helpers of the GPU parity tests: run the CUDA path (through the C ABI binding) and the
+CPU oracle on the same seeded inputs and compare them element by element.
+
+Tolerances are BASELINE.json north_star's: P codes identical >= 99.99 % (isolation) / >= 99.9 %
+(FP8 mode); output relative L2 <= 1e-3 / <= 2e-2; MSE against the unquantised FP64 reference
+within 10 % of the oracle's MSE.  row_max at atol 1e-5, row_sum at rtol 1e-5.
+"""
+from dataclasses import dataclass
+
+import numpy as np
+import torch
+
+import oracle
+from paper_2606_06521_b200 import workloads as W
+
+CODE_MATCH = {1: 0.9999, 2: 0.999}
+REL_L2 = {0: 1e-5, 1: 1e-3, 2: 2e-2}
+
+
+def fa():
+    from paper_2606_06521_b200 import fp8attn
+    return fp8attn
+
+
+def dev():
+    return torch.device("cuda:0")
+
+
+def to_dev(a: np.ndarray, bf16=False):
+    t = torch.from_numpy(np.ascontiguousarray(a)).to(dev())
+    return t.view(torch.bfloat16) if bf16 else t
+
+
+@dataclass
+class Case:
+    q: np.ndarray          # oracle-side arrays (float32 / uint16 BF16 bits / uint8 E4M3 codes)
+    k: np.ndarray
+    v: np.ndarray
+    in_dtype: int          # oracle.DT_*
+    tq: torch.Tensor       # device tensors for the CUDA path
+    tk: torch.Tensor
+    tv: torch.Tensor
+    scales: dict           # q_scale/k_scale/v_scale numpy (oracle) -- same values on device
+
+
+def make_case(q, k, v, kind: str) -> Case:
+    """kind: 'f32' | 'bf16' | 'e4m3' (all three quantised by the oracle-side helper, so no input
+    of the oracle comes from the CUDA path) | 'decode' (BF16 q, E4M3 k/v)."""
+    if kind == "f32":
+        return Case(q, k, v, oracle.DT_F32, to_dev(q), to_dev(k), to_dev(v), {})
+    if kind == "bf16":
+        qb, kb, vb = W.to_bf16_bits(q), W.to_bf16_bits(k), W.to_bf16_bits(v)
+        return Case(qb, kb, vb, oracle.DT_BF16, to_dev(qb, True), to_dev(kb, True), to_dev(vb, True), {})
+    kc, ks = oracle.quantize_e4m3(k)
+    vc, vs = oracle.quantize_e4m3(v)
+    if kind == "e4m3":
+        qc, qs = oracle.quantize_e4m3(q)
+        sc = {"q_scale": qs, "k_scale": ks, "v_scale": vs}
+        return Case(qc, kc, vc, oracle.DT_E4M3, to_dev(qc), to_dev(kc), to_dev(vc), sc)
+    if kind == "decode":
+        qb = W.to_bf16_bits(q)
+        sc = {"k_scale": ks, "v_scale": vs}
+        return Case(qb, kc, vc, oracle.DT_BF16Q_E4M3KV, to_dev(qb, True), to_dev(kc), to_dev(vc), sc)
+    raise ValueError(kind)
+
+
+def run_gpu(case: Case, *, causal, S, order, mode, block_n=0, num_splits=0, n_sink=4, stats=True, dump_head=None):
+    f = fa()
+    sc = {n: torch.from_numpy(a).to(dev()) for n, a in case.scales.items()}
+    r = f.fwd(case.tq, case.tk, case.tv, causal=causal, S=S, kv_order=order, mode=mode, n_sink=n_sink,
+              block_n=block_n, num_splits=num_splits, want_stats=stats, dump_head=dump_head, **sc)
+    torch.cuda.synchronize()
+    return r
+
+
+def run_oracle(case: Case, r, *, causal, S, order, mode, n_sink=4, rows=None, want_codes=False):
+    """Oracle on the same inputs, mirroring the tiling the library reports (block_n, split bounds)."""
+    return oracle.attention_fwd(case.q, case.k, case.v, causal=causal, S=S, kv_order=order, mode=mode,
+                                in_dtype=case.in_dtype, block_n=r.block_n, n_sink=n_sink,
+                                split_bounds=r.split_bounds if r.num_splits > 1 else None,
+                                rows=rows, want_codes=want_codes, **case.scales)
+
+
+def rel_l2(a, b):
+    den = np.linalg.norm(b)
+    return float(np.linalg.norm(a - b) / den) if den > 0 else float(np.linalg.norm(a - b))
+
+
+def check(case: Case, r, ref, *, mode, rows=None, codes_rows=None, label="", check_mse=True, check_uf=True):
+    """Compare one GPU result with the oracle result on `rows` (flat row ids; None = all)."""
+    d = case.tq.shape[-1]
+    o = r.o.detach().cpu().numpy().reshape(-1, d).astype(np.float64)
+    if rows is not None:
+        o = o[rows]
+    err = rel_l2(o, ref.out)
+    assert err <= REL_L2[mode], f"{label}: output rel-L2 {err:.3e} > {REL_L2[mode]}"
+    out = {"rel_l2": err}
+    if r.row_max is not None:
+        rm = r.row_max.cpu().numpy().reshape(-1)
+        rs = r.row_sum.cpu().numpy().reshape(-1).astype(np.float64)
+        if rows is not None:
+            rm, rs = rm[rows], rs[rows]
+        fin = np.isfinite(ref.row_max)
+        assert np.array_equal(np.isfinite(rm), fin), f"{label}: row_max finiteness"
+        tol = 1e-5 if mode != 2 else 1e-4
+        assert np.allclose(rm[fin], ref.row_max[fin], rtol=tol, atol=tol), \
+            f"{label}: row_max max diff {np.abs(rm[fin] - ref.row_max[fin]).max():.3e}"
+        rtol = 1e-5 if mode != 2 else 1e-3
+        assert np.allclose(rs, ref.row_sum, rtol=rtol, atol=0), \
+            f"{label}: row_sum max rel diff {np.max(np.abs(rs - ref.row_sum) / np.maximum(ref.row_sum, 1e-30)):.3e}"
+    n_flip = None
+    if r.p_codes is not None and ref.p_codes is not None and mode != 0:
+        g = r.p_codes.cpu().numpy()
+        if codes_rows is not None:
+            g = g[codes_rows]
+        assert np.array_equal(g == 0xFF, ref.p_codes == 0xFF), f"{label}: mask pattern of the P dump differs"
+        vis = ref.p_codes != 0xFF
+        n_flip = int(np.sum(g[vis] != ref.p_codes[vis]))
+        match = 1.0 - n_flip / max(1, int(vis.sum()))
+        assert match >= CODE_MATCH[mode], f"{label}: P code match {match:.6f} < {CODE_MATCH[mode]}"
+        # a flip moves a code by exactly one step
+        dd = np.abs(g[vis].astype(np.int32) - ref.p_codes[vis].astype(np.int32))
+        assert dd.max(initial=0) <= 1, f"{label}: a P code differs by more than one step"
+        out["code_match"] = match
+    if check_uf and r.underflow is not None and mode != 0 and rows is None:
+        uf = r.underflow.cpu().numpy()
+        slack = max(4, int(2e-4 * ref.n_nonsink_visible) if mode == 1 else int(2e-3 * ref.n_nonsink_visible))
+        if n_flip is not None and case.tq.shape[0] * case.tq.shape[1] == 1:
+            slack = n_flip      # the dump covers every P: counters can differ only where codes flipped
+        assert abs(int(uf[0]) - ref.uf_sink_block) <= slack, f"{label}: sink-block underflow {uf[0]} vs {ref.uf_sink_block}"
+        assert abs(int(uf[1]) - ref.uf_other_blocks) <= slack, f"{label}: other-block underflow {uf[1]} vs {ref.uf_other_blocks}"
+        out["underflow"] = (int(uf[0]), int(uf[1]))
+    if check_mse and mode != 0:
+        mse_gpu = float(np.mean((o - ref.ref) ** 2))
+        assert abs(mse_gpu - ref.mse) <= 0.10 * ref.mse + 1e-14, f"{label}: MSE gpu {mse_gpu:.4e} oracle {ref.mse:.4e}"
+        out["mse"] = (mse_gpu, ref.mse)
+    return out
