@@ -77,7 +77,7 @@ static uint8_t round_e4m3_pos(double x)
     if (!(x > 0.0))
         return 0;
     if (x >= 448.0)
-        return 0x7E;                              /* satfinite, reading R9 */
+        return 0x7E;                              /* satfinite, reading R22 */
     int lo = 0;                                   /* largest code with value <= x */
     for (int c = 1; c <= 0x7E; ++c) {
         if (e4m3_code_value(c) <= x)
@@ -245,7 +245,7 @@ static void attend_row(const problem *P, int64_t rid, int64_t sel,
         for (int t = 0; t < d; ++t) qv[t] *= (double)o->q_scale[bh];
     } else if (o->in_dtype == DT_BF16Q_E4M3KV) {
         /* decode: q is BF16 in memory and is quantised to E4M3 per (b,hq) slab
-         * before use (reading R8 / DESIGN.md); the input VALUES of the method are
+         * before use (reading R24 / DESIGN.md); the input VALUES of the method are
          * the post-quantisation ones. */
         float *qf = (float *)malloc(sizeof(float) * (size_t)Lq * d);
         uint8_t *qc = (uint8_t *)malloc((size_t)Lq * d);

@@ -266,7 +266,7 @@ int fp8attn_fwd(const void* q, const void* k, const void* v, void* o, int B, int
     } else if (dt == 2) {
         eb = 1;
     } else if (dt == 3) {
-        // decode: quantise the BF16 q of every (b, hq) slab to E4M3 (reading R8 in DESIGN.md)
+        // decode: quantise the BF16 q of every (b, hq) slab to E4M3 (reading R24 in DESIGN.md)
         eb = 1;
         void *wq = nullptr, *wa = nullptr;
         if (int rc = g_qquant.get(&wq, (size_t)nq + (size_t)q_slabs * 4 + 16, st)) return rc;

@@ -133,7 +133,7 @@ def test_ragged_shapes(shape, kind, mode, order):
 # ------------------------------------------------------------------ S values incl. saturation
 @pytest.mark.parametrize("S", [1.0, 16.0, 448.0, 512.0, 3.0])
 def test_scale_values(S):
-    """448 (not a power of two: double rounding of fl32(p*S)) and 512 (satfinite at 448, reading R9)."""
+    """448 (not a power of two: double rounding of fl32(p*S)) and 512 (satfinite at 448, reading R22)."""
     q, k, v = W.sink_qkv(1, 2, 2, 256, 256, 128, 9.0, seed=2)
     case = P.make_case(q, k, v, "f32")
     r = P.run_gpu(case, causal=False, S=S, order=0, mode=1, block_n=64, dump_head=(0, 1))

@@ -211,7 +211,7 @@ def test_bf16_and_e4m3_inputs_equal_fp32_of_same_values():
 
 
 def test_decode_dtype_quantises_q_per_head():
-    """BF16 q + E4M3 KV: q is quantised per (b,hq) slab (reading R8)."""
+    """BF16 q + E4M3 KV: q is quantised per (b,hq) slab (reading R24)."""
     rng = np.random.default_rng(9)
     B, Hq, Hkv, Lk, d = 2, 4, 2, 96, 16
     q = rng.standard_normal((B, Hq, 1, d)).astype(np.float32)

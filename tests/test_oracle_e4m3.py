@@ -62,7 +62,7 @@ def test_round_ties_and_thresholds(golden):
     assert oracle.round_e4m3(2.5 * 2.0 ** -9) == 2             # tie 2|3 -> 2
     assert oracle.round_e4m3(7.5 * 2.0 ** -9) == 8             # tie 7|8 -> min normal 2^-6
     assert oracle.round_e4m3(448.0) == 0x7E
-    assert oracle.round_e4m3(1e9) == 0x7E                      # satfinite (reading R9)
+    assert oracle.round_e4m3(1e9) == 0x7E                      # satfinite (reading R22)
     assert oracle.round_e4m3(float("inf")) == 0x7E
     assert oracle.round_e4m3(0.0) == 0 and oracle.round_e4m3(-0.0) == 0x80
     assert oracle.round_e4m3(-1.0) == (0x80 | oracle.round_e4m3(1.0))
