@@ -76,6 +76,10 @@ typedef struct fp8attn_stats {
                                   ("typically 64 or 128")                          */
     int32_t num_splits;        /* split-KV request: 0 = automatic, n >= 1 = exactly n contiguous
                                   block ranges                             */
+    int32_t kernel;            /* kernel family request: 0 = automatic, 1 = general kernel, 2 = warp-
+                                  specialised prefill kernel, 3 = split-KV decode kernel; a family
+                                  that cannot serve the call gives FP8ATTN_E_UNSUPPORTED       */
+    int32_t reserved0;         /* must be 0                                                      */
     const float *q_scale;      /* device [B*Hq]  dequantisation scale of E4M3 q (value = code*scale) */
     const float *k_scale;      /* device [B*Hkv]                                                 */
     const float *v_scale;      /* device [B*Hkv]                                                 */

@@ -9,6 +9,7 @@
 
 #include "../../include/fp8attn.h"
 #include "attn_general.cuh"
+#include "attn_prefill.cuh"
 #include "debug_gemm.cuh"
 #include "prep.cuh"
 
@@ -159,6 +160,29 @@ int dispatch_general(int d, int bn, const CUtensorMap& mq, const CUtensorMap& mk
     return FP8ATTN_E_UNSUPPORTED;
 }
 
+// ---------------------------------------------------------------------------- prefill kernel launch
+template <int EB, bool FOLD>
+int launch_prefill(const CUtensorMap& mq, const CUtensorMap& mk, const CUtensorMap& mv, const FwdParams& p,
+                   cudaStream_t st) {
+    using C = PrefillCfg<EB>;
+    auto kern = attn_prefill_kernel<EB, FOLD>;
+    static bool configured = false;
+    if (!configured) {
+        CU_TRY(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, C::SMEM_BYTES));
+        configured = true;
+    }
+    const dim3 grid((unsigned)((p.Lq + 2 * BM - 1) / (2 * BM)), (unsigned)(p.B * p.Hq));
+    kern<<<grid, C::THREADS, C::SMEM_BYTES, st>>>(mq, mk, mv, p);
+    CU_TRY(cudaGetLastError());
+    return FP8ATTN_OK;
+}
+
+// S = 2^k with a comfortable exponent: the factor can be folded into the exponent of P exactly
+bool is_pow2_scale(float S) {
+    int e = 0;
+    return std::frexp(S, &e) == 0.5f && e > -20 && e < 20;
+}
+
 // Argument checks shared by fp8attn_fwd and fp8attn_fwd_host: no CUDA call before these pass.
 int validate_args(const void* q, const void* k, const void* v, const void* o, int B, int Hq, int Hkv, int Lq, int Lk,
                   int d, float S, int kv_order, int mode, const fp8attn_stats* stats) {
@@ -182,6 +206,7 @@ int validate_args(const void* q, const void* k, const void* v, const void* o, in
     if (dt == 0 && bn == 128) return FP8ATTN_E_UNSUPPORTED;
     const int ns = stats ? stats->num_splits : 0;
     if (ns < 0 || ns > FP8ATTN_MAX_SPLITS) return FP8ATTN_E_UNSUPPORTED;
+    if (stats && (stats->kernel < 0 || stats->kernel > 3 || stats->reserved0 != 0)) return FP8ATTN_E_MODE;
     if (stats && stats->p_codes && (stats->p_batch < 0 || stats->p_batch >= B || stats->p_head < 0 || stats->p_head >= Hq))
         return FP8ATTN_E_SHAPE;
     if ((long long)B * Hq > 65535) return FP8ATTN_E_UNSUPPORTED;
@@ -322,9 +347,23 @@ int fp8attn_fwd(const void* q, const void* k, const void* v, void* o, int B, int
     }
     if (p.underflow) CU_TRY(cudaMemsetAsync(p.underflow, 0, 2 * sizeof(unsigned long long), st));
 
+    // kernel family: the warp-specialised prefill kernel serves d = 128, Bn = 128, one split, BF16 or
+    // E4M3 operands, modes 1 and 2, when neither the P dump nor the underflow counters are asked for.
+    const int want_kernel = stats ? stats->kernel : 0;
+    const bool prefill_ok = d == 128 && bn == 128 && ns == 1 && npl == 1 && pm != 0 && dt != 3 && !p.p_codes &&
+                            !p.underflow;
+    if (want_kernel == 2 && !prefill_ok) return FP8ATTN_E_UNSUPPORTED;
+    if (want_kernel == 3) return FP8ATTN_E_UNSUPPORTED;
+    const bool use_prefill = prefill_ok && (want_kernel == 2 || (want_kernel == 0 && Lq > 16));
+    int kernel_id = 1;
     const dim3 grid((unsigned)n_qtiles, (unsigned)q_slabs, (unsigned)ns);
     int rc;
-    if (npl == 3)
+    if (use_prefill) {
+        kernel_id = 2;
+        const bool fold = is_pow2_scale(S);
+        if (eb == 1) rc = fold ? launch_prefill<1, true>(mq, mk, mv, p, st) : launch_prefill<1, false>(mq, mk, mv, p, st);
+        else rc = fold ? launch_prefill<2, true>(mq, mk, mv, p, st) : launch_prefill<2, false>(mq, mk, mv, p, st);
+    } else if (npl == 3)
         rc = (pm == 0) ? dispatch_general<2, 3, 0>(d, bn, mq, mk, mv, p, grid, st)
                        : dispatch_general<2, 3, 1>(d, bn, mq, mk, mv, p, grid, st);
     else if (eb == 2)
@@ -343,11 +382,11 @@ int fp8attn_fwd(const void* q, const void* k, const void* v, void* o, int B, int
         ++n_launches;
     }
     if (stats) {
-        stats->block_m_used = BM;
+        stats->block_m_used = (kernel_id == 2) ? 2 * BM : BM;
         stats->block_n_used = bn;
         stats->num_splits_used = ns;
         for (int s = 0; s <= ns; ++s) stats->split_bounds[s] = (int)(((long long)s * nb) / ns);
-        stats->kernel_id = 1;
+        stats->kernel_id = kernel_id;
         stats->n_launches = n_launches;
     }
     return FP8ATTN_OK;

@@ -25,7 +25,7 @@ class Stats(C.Structure):
     """struct fp8attn_stats"""
     _fields_ = [
         ("struct_size", C.c_int32), ("n_sink", C.c_int32), ("block_n", C.c_int32),
-        ("num_splits", C.c_int32),
+        ("num_splits", C.c_int32), ("kernel", C.c_int32), ("reserved0", C.c_int32),
         ("q_scale", C.c_void_p), ("k_scale", C.c_void_p), ("v_scale", C.c_void_p),
         ("stream", C.c_void_p), ("p_codes", C.c_void_p),
         ("p_batch", C.c_int32), ("p_head", C.c_int32),
@@ -121,11 +121,13 @@ def _dtype_code(q, k):
 
 
 def fwd(q, k, v, *, causal: bool, S: float, kv_order: int, mode: int, n_sink: int = 4,
-        block_n: int = 0, num_splits: int = 0, q_scale=None, k_scale=None, v_scale=None,
-        want_stats: bool = False, dump_head=None, out=None, stream=None) -> FwdResult:
+        block_n: int = 0, num_splits: int = 0, kernel: int = 0, q_scale=None, k_scale=None, v_scale=None,
+        want_stats: bool = False, want_underflow: Optional[bool] = None, dump_head=None, out=None,
+        stream=None) -> FwdResult:
     """fp8attn_fwd on CUDA tensors q [B,Hq,Lq,d], k/v [B,Hkv,Lk,d] (contiguous).  `mode` is the
     P mode (0 no-cast, 1 isolation, 2 FP8); the input dtype bits are derived from the tensors.
-    `dump_head=(b,h)` returns the E4M3 code of every P of that head."""
+    `dump_head=(b,h)` returns the E4M3 code of every P of that head.  `kernel` requests a kernel
+    family (0 automatic; the P dump and the underflow counters exist in the general kernel only)."""
     for t in (q, k, v):
         if not (t.is_cuda and t.is_contiguous() and t.dim() == 4):
             raise ValueError("q, k, v must be contiguous 4-D CUDA tensors")
@@ -136,7 +138,7 @@ def fwd(q, k, v, *, causal: bool, S: float, kv_order: int, mode: int, n_sink: in
     o = out if out is not None else torch.empty((B, Hq, Lq, d), dtype=torch.float32, device=q.device)
     st = Stats()
     st.struct_size = C.sizeof(Stats)
-    st.n_sink, st.block_n, st.num_splits = n_sink, block_n, num_splits
+    st.n_sink, st.block_n, st.num_splits, st.kernel = n_sink, block_n, num_splits, kernel
     st.stream = _stream_ptr(stream)
     keep = []
     for name, t in (("q_scale", q_scale), ("k_scale", k_scale), ("v_scale", v_scale)):
@@ -148,8 +150,10 @@ def fwd(q, k, v, *, causal: bool, S: float, kv_order: int, mode: int, n_sink: in
     if want_stats:
         row_max = torch.empty((B, Hq, Lq), dtype=torch.float32, device=q.device)
         row_sum = torch.empty((B, Hq, Lq), dtype=torch.float32, device=q.device)
+        st.row_max, st.row_sum = row_max.data_ptr(), row_sum.data_ptr()
+    if want_stats if want_underflow is None else want_underflow:
         underflow = torch.zeros(2, dtype=torch.int64, device=q.device)
-        st.row_max, st.row_sum, st.underflow = row_max.data_ptr(), row_sum.data_ptr(), underflow.data_ptr()
+        st.underflow = underflow.data_ptr()
     if dump_head is not None:
         codes = torch.full((Lq, Lk), 0xFF, dtype=torch.uint8, device=q.device)
         st.p_codes = codes.data_ptr()
@@ -164,8 +168,9 @@ def fwd(q, k, v, *, causal: bool, S: float, kv_order: int, mode: int, n_sink: in
 
 
 def fwd_host(q, k, v, *, causal: bool, S: float, kv_order: int, mode: int, n_sink: int = 4,
-             block_n: int = 0, num_splits: int = 0, q_scale=None, k_scale=None, v_scale=None,
-             want_stats: bool = False, out=None, stream=None, device=None) -> FwdResult:
+             block_n: int = 0, num_splits: int = 0, kernel: int = 0, q_scale=None, k_scale=None, v_scale=None,
+             want_stats: bool = False, want_underflow: Optional[bool] = None, out=None, stream=None,
+             device=None) -> FwdResult:
     """fp8attn_fwd_host on HOST tensors (CPU, ideally pinned): the library copies them to the
     device, runs the kernels, copies `o` (and statistics) back and synchronises the stream."""
     for t in (q, k, v):
@@ -178,7 +183,7 @@ def fwd_host(q, k, v, *, causal: bool, S: float, kv_order: int, mode: int, n_sin
     o = out if out is not None else torch.empty((B, Hq, Lq, d), dtype=torch.float32, pin_memory=True)
     st = Stats()
     st.struct_size = C.sizeof(Stats)
-    st.n_sink, st.block_n, st.num_splits = n_sink, block_n, num_splits
+    st.n_sink, st.block_n, st.num_splits, st.kernel = n_sink, block_n, num_splits, kernel
     keep = []
     for name, t in (("q_scale", q_scale), ("k_scale", k_scale), ("v_scale", v_scale)):
         if t is not None:
@@ -189,8 +194,10 @@ def fwd_host(q, k, v, *, causal: bool, S: float, kv_order: int, mode: int, n_sin
     if want_stats:
         row_max = torch.empty((B, Hq, Lq), dtype=torch.float32, pin_memory=True)
         row_sum = torch.empty((B, Hq, Lq), dtype=torch.float32, pin_memory=True)
+        st.row_max, st.row_sum = row_max.data_ptr(), row_sum.data_ptr()
+    if want_stats if want_underflow is None else want_underflow:
         underflow = torch.zeros(2, dtype=torch.int64, pin_memory=True)
-        st.row_max, st.row_sum, st.underflow = row_max.data_ptr(), row_sum.data_ptr(), underflow.data_ptr()
+        st.underflow = underflow.data_ptr()
     dev = torch.device("cuda", torch.cuda.current_device()) if device is None else torch.device(device)
     with torch.cuda.device(dev):
         st.stream = _stream_ptr(stream)

@@ -64,11 +64,15 @@ def make_case(q, k, v, kind: str) -> Case:
     raise ValueError(kind)
 
 
-def run_gpu(case: Case, *, causal, S, order, mode, block_n=0, num_splits=0, n_sink=4, stats=True, dump_head=None):
+def run_gpu(case: Case, *, causal, S, order, mode, block_n=0, num_splits=0, n_sink=4, stats=True, dump_head=None,
+            kernel=0, underflow=None):
+    """kernel: 0 automatic, 1 general, 2 prefill, 3 decode.  underflow=False keeps row_max / row_sum but
+    not the underflow counters (which only the general kernel carries)."""
     f = fa()
     sc = {n: torch.from_numpy(a).to(dev()) for n, a in case.scales.items()}
     r = f.fwd(case.tq, case.tk, case.tv, causal=causal, S=S, kv_order=order, mode=mode, n_sink=n_sink,
-              block_n=block_n, num_splits=num_splits, want_stats=stats, dump_head=dump_head, **sc)
+              block_n=block_n, num_splits=num_splits, kernel=kernel, want_stats=stats, want_underflow=underflow,
+              dump_head=dump_head, **sc)
     torch.cuda.synchronize()
     return r
 
