@@ -2,9 +2,12 @@
 //
 // One CTA = two 128-row query tiles (256 consecutive query rows) of one (batch, q head).  Roles:
 //   warps 0-3  softmax of tile 0      warps 4-7  softmax of tile 1   (one query row per thread = TMEM lane)
-//   warp  8    tcgen05.mma issuer     warp  9    TMA producer
+//   warps 8, 9 tcgen05.mma issuers of tile 0 / tile 1     warp 10  TMA producer
 // TMEM (512 columns): S0 [0,128) S1 [128,256) O0 [256,384) O1 [384,512); P_t is written over the first
-// 32 (E4M3) / 64 (BF16) columns of S_t and read from there as the A operand of O_t += P_t V.
+// head of each 32-column quarter of S_t (8 columns E4M3 / 16 BF16) and read from there as the A operand
+// of O_t += P_t V.  S and P move in quarters: QK^T is issued as four N = 32 MMAs groups, P.V as four K = 32
+// groups, each with its own mbarrier, so the tensor pipe works on quarter q while the softmax warps are
+// still on quarter q+1 and the serial chain exp -> P.V -> QK^T -> max shrinks to one quarter.
 // The tensor pipe executes in issue order: ... PV_0(j), QK_0(j+1), PV_1(j), QK_1(j+1) ..., so while the
 // softmax warps of tile 0 work on S_0(j+1) the tensor core runs tile 1 and vice versa; the two softmax
 // groups share the MUFU pipe, which is the binding unit (16 ex2 / clk / SM against 16384 FP8 FLOP / clk).
@@ -28,11 +31,11 @@ struct PrefillCfg {
     static constexpr int KSTEP = 32 / EB;            // contraction elements per MMA
     static constexpr int P_COLS = BN * EB / 4;       // TMEM columns of P
     static constexpr int TM_S = 0, TM_O = 256;
-    static constexpr int N_BARS = 2 + 4 * NS + 6;
+    static constexpr int N_BARS = 2 + 4 * NS + 8 + 8 + 2;
     static constexpr int SMEM_BYTES = (2 + 2 * NS) * TILE + 1024 /*align*/ + N_BARS * 8 + 16;
     static constexpr uint32_t KIND = (EB == 1) ? ptx::KIND_F8F6F4 : ptx::KIND_F16;
     static constexpr uint32_t FMT = (EB == 1) ? ptx::FMT_E4M3 : ptx::FMT_BF16;
-    static constexpr int THREADS = 320;
+    static constexpr int THREADS = 352;
 };
 
 // exact E4M3 pair -> BF16 pair: the code shifted left by 4 is the BF16 bit pattern of value * 2^-120
@@ -92,7 +95,7 @@ __device__ __forceinline__ void exp_chunk(const uint32_t* v, uint32_t* w, int j_
 }
 
 // ---- softmax warpgroup: all of Alg. 1 lines 4-9 and 12 for one 128-row tile ----------------------
-template <int EB, bool FOLD>
+template <int EB, bool FOLD, int QKG>
 __device__ __forceinline__ void prefill_softmax(const FwdParams& p, int t, int wq, int lane, uint32_t tbase,
                                                 uint64_t* s_full, uint64_t* p_full, uint64_t* o_done, int n_t,
                                                 int row0, int bh, int kvh) {
@@ -122,18 +125,27 @@ __device__ __forceinline__ void prefill_softmax(const FwdParams& p, int t, int w
         const int blk = (p.kv_order == 0) ? c : n_t - 1 - c;
         const int j0 = blk * C::BN;
         const bool mask = (j0 + C::BN - 1 > warp_vis) || (j0 + C::BN > p.Lk);
-        ptx::mbar_wait(s_full, c & 1);
-        ptx::tc_fence_after();
-
-        // ---- lines 4-5: block max, running max ----
+        // ---- lines 4-5: block max, running max.  S arrives in four 32-column quarters ----
         float mloc = -INFINITY;
         {
             uint32_t va[32], vb[32];
-            ptx::tmem_ld_x32(tS, va);
-            ptx::tmem_ld_x32(tS + 32, vb);
-            ptx::tmem_wait_ld();
 #pragma unroll
             for (int h = 0; h < 2; ++h) {
+                if constexpr (QKG == 4) {
+                    ptx::mbar_wait(s_full + 2 * h, c & 1);
+                    ptx::tc_fence_after();
+                    ptx::tmem_ld_x32(tS + h * 64, va);
+                    ptx::mbar_wait(s_full + 2 * h + 1, c & 1);
+                    ptx::tc_fence_after();
+                } else {
+                    if (QKG == 2 || h == 0) {
+                        ptx::mbar_wait(s_full + (QKG == 2 ? h : 0), c & 1);
+                        ptx::tc_fence_after();
+                    }
+                    ptx::tmem_ld_x32(tS + h * 64, va);
+                }
+                ptx::tmem_ld_x32(tS + h * 64 + 32, vb);
+                ptx::tmem_wait_ld();
                 if (mask) {
 #pragma unroll
                     for (int e = 0; e < 32; ++e) {
@@ -148,11 +160,6 @@ __device__ __forceinline__ void prefill_softmax(const FwdParams& p, int t, int w
                     m1 = fmaxf(fmaxf(m1, __uint_as_float(vb[e])), __uint_as_float(vb[e + 1]));
                 }
                 mloc = fmaxf(m0, m1);
-                if (h == 0) {
-                    ptx::tmem_ld_x32(tS + 64, va);
-                    ptx::tmem_ld_x32(tS + 96, vb);
-                    ptx::tmem_wait_ld();
-                }
             }
         }
         const float m_new = fmaxf(m_run, mloc);
@@ -165,18 +172,20 @@ __device__ __forceinline__ void prefill_softmax(const FwdParams& p, int t, int w
         if (c > 0 && __any_sync(0xFFFFFFFFu, alpha != 1.0f)) {
             const uint64_t a2 = ptx::pack2(alpha, alpha);
 #pragma unroll 1
-            for (int cb = 0; cb < 4; ++cb) {
-                uint32_t v[32];
-                ptx::tmem_ld_x32(tO + cb * 32, v);
+            for (int hb = 0; hb < 2; ++hb) {
+                uint32_t v[64];
+                ptx::tmem_ld_x32(tO + hb * 64, v);
+                ptx::tmem_ld_x32(tO + hb * 64 + 32, v + 32);
                 ptx::tmem_wait_ld();
 #pragma unroll
-                for (int e = 0; e < 32; e += 2) {
+                for (int e = 0; e < 64; e += 2) {
                     float y0, y1;
                     ptx::unpack2(ptx::mul2(ptx::pack2u(v[e], v[e + 1]), a2), y0, y1);
                     v[e] = __float_as_uint(y0);
                     v[e + 1] = __float_as_uint(y1);
                 }
-                ptx::tmem_st_x32(tO + cb * 32, v);
+                ptx::tmem_st_x32(tO + hb * 64, v);
+                ptx::tmem_st_x32(tO + hb * 64 + 32, v + 32);
             }
         }
 
@@ -195,15 +204,16 @@ __device__ __forceinline__ void prefill_softmax(const FwdParams& p, int t, int w
                     exp_chunk<EB, FOLD, true>(cur, w, j0 + cb * 32, jlim, cl2_2, negm_2, s_2, sum_a, sum_b);
                 else
                     exp_chunk<EB, FOLD, false>(cur, w, j0 + cb * 32, jlim, cl2_2, negm_2, s_2, sum_a, sum_b);
+                // P quarter over the head of its own S quarter; the P.V of this quarter can start at once
+                if constexpr (EB == 1) ptx::tmem_st_x8(tS + cb * 32, w);
+                else ptx::tmem_st_x16(tS + cb * 32, w);
+                ptx::tmem_wait_st();       // (also covers the O rescale stores before the first quarter)
+                ptx::tc_fence_before();
+                __syncwarp();
+                if (lane == 0) ptx::mbar_arrive(p_full + cb);
                 if (cb < 3) ptx::tmem_wait_ld();
-                if constexpr (EB == 1) ptx::tmem_st_x8(tS + cb * 8, w);
-                else ptx::tmem_st_x16(tS + cb * 16, w);
             }
         }
-        ptx::tmem_wait_st();
-        ptx::tc_fence_before();
-        __syncwarp();
-        if (lane == 0) ptx::mbar_arrive(p_full);
         float sa, sb, sc, sd;
         ptx::unpack2(sum_a, sa, sb);
         ptx::unpack2(sum_b, sc, sd);
@@ -248,8 +258,8 @@ __device__ __forceinline__ void prefill_softmax(const FwdParams& p, int t, int w
 
 // ---- the kernel ---------------------------------------------------------------------------------
 // grid = (ceil(Lq / 256), B*Hq).  Causal launches the heaviest tile pairs first.
-template <int EB, bool FOLD>
-__global__ void __launch_bounds__(320, 1)
+template <int EB, bool FOLD, int QKG>
+__global__ void __launch_bounds__(352, 1)
 attn_prefill_kernel(const __grid_constant__ CUtensorMap mapQ, const __grid_constant__ CUtensorMap mapK,
                     const __grid_constant__ CUtensorMap mapV, const FwdParams p) {
     using C = PrefillCfg<EB>;
@@ -264,12 +274,13 @@ attn_prefill_kernel(const __grid_constant__ CUtensorMap mapQ, const __grid_const
     uint64_t* k_empty = k_full + C::NS;
     uint64_t* v_full = k_empty + C::NS;
     uint64_t* v_empty = v_full + C::NS;
-    uint64_t* s_full = v_empty + C::NS;           // [2]
-    uint64_t* p_full = s_full + 2;                // [2]
-    uint64_t* o_done = p_full + 2;                // [2]
+    uint64_t* s_full = v_empty + C::NS;           // [2 tiles][4 quarters]  MMA -> softmax
+    uint64_t* p_full = s_full + 8;                // [2 tiles][4 quarters]  softmax (4 warps) -> MMA
+    uint64_t* o_done = p_full + 8;                // [2]
     uint32_t* tmem_slot = reinterpret_cast<uint32_t*>(o_done + 2);
 
-    const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
+    const int tid = threadIdx.x, lane = tid & 31;
+    const int warp = __shfl_sync(0xFFFFFFFFu, tid >> 5, 0);   // provably warp-uniform
     const int pair = p.causal ? (int)(gridDim.x - 1 - blockIdx.x) : (int)blockIdx.x;
     const int bh = blockIdx.y;
     const int b = bh / p.Hq, h = bh % p.Hq;
@@ -297,11 +308,17 @@ attn_prefill_kernel(const __grid_constant__ CUtensorMap mapQ, const __grid_const
         ptx::prefetch_tmap(&mapQ);
         ptx::prefetch_tmap(&mapK);
         ptx::prefetch_tmap(&mapV);
-        for (int i = 0; i < 2 + 4 * C::NS; ++i) ptx::mbar_init(bars + i, 1);
-        ptx::mbar_init(s_full + 0, 1);
-        ptx::mbar_init(s_full + 1, 1);
-        ptx::mbar_init(p_full + 0, 4);
-        ptx::mbar_init(p_full + 1, 4);
+        for (int i = 0; i < 2; ++i) ptx::mbar_init(q_full + i, 1);
+        for (int i = 0; i < C::NS; ++i) {
+            ptx::mbar_init(k_full + i, 1);
+            ptx::mbar_init(v_full + i, 1);
+            ptx::mbar_init(k_empty + i, 2);   // one arrival per tile
+            ptx::mbar_init(v_empty + i, 2);
+        }
+        for (int i = 0; i < 8; ++i) {
+            ptx::mbar_init(s_full + i, 1);
+            ptx::mbar_init(p_full + i, 4);
+        }
         ptx::mbar_init(o_done + 0, 1);
         ptx::mbar_init(o_done + 1, 1);
         ptx::fence_mbar_init();
@@ -317,9 +334,9 @@ attn_prefill_kernel(const __grid_constant__ CUtensorMap mapQ, const __grid_const
 
     if (warp < 8) {
         const int t = warp >> 2;
-        prefill_softmax<EB, FOLD>(p, t, warp & 3, lane, tbase, s_full + t, p_full + t, o_done + t, n_tile[t],
-                                  (pair * 2 + t) * BM, bh, kvh);
-    } else if (warp == 9) {
+        prefill_softmax<EB, FOLD, QKG>(p, t, warp & 3, lane, tbase, s_full + 4 * t, p_full + 4 * t, o_done + t,
+                                  n_tile[t], (pair * 2 + t) * BM, bh, kvh);
+    } else if (warp == 10) {
         // ================= TMA producer =================
         if (lane == 0 && n_it > 0) {
             for (int t = 0; t < 2; ++t) {
@@ -345,76 +362,91 @@ attn_prefill_kernel(const __grid_constant__ CUtensorMap mapQ, const __grid_const
                                      blk * C::BN, kvh);
             }
         }
-    } else if (lane == 0 && n_it > 0) {
-        // ================= MMA issuer (one thread) =================
-        constexpr uint32_t idesc_qk = ptx::make_idesc(C::FMT, C::FMT, ptx::MAJOR_K, ptx::MAJOR_K, BM, C::BN);
+    } else if (n_tile[warp - 8] > 0) {
+        // ================= MMA issuer of tile t = warp - 8 =================
+        // One issuer warp per tile, each blocking only on its own tile's barriers and on the K/V ring, so
+        // neither tile can hold up the other.  The whole warp runs the loop (warp-uniform control flow keeps
+        // descriptors and counters in uniform registers); one elected lane issues the MMAs and commits.
+        // Block c of tile t uses K/V ring iteration it = c + first (in reverse order the tile with fewer
+        // visible blocks joins later).  A ring slot is released by two arrivals, one per tile; on iterations
+        // that only one tile uses, that tile arrives twice.
+        const int t = warp - 8;
+        const int n_t = n_tile[t];
+        const bool leader = ptx::elect_one();
+        constexpr int NG = 128 / QKG;          // keys per QK^T group
+        constexpr int QPG = 4 / QKG;           // P quarters per QK^T group
+        constexpr uint32_t idesc_qk = ptx::make_idesc(C::FMT, C::FMT, ptx::MAJOR_K, ptx::MAJOR_K, BM, NG);
         constexpr uint32_t idesc_pv = ptx::make_idesc(C::FMT, C::FMT, ptx::MAJOR_K, ptx::MAJOR_MN, BM, C::D);
-        // tile t takes part in iteration it iff its block is visible to it
-        auto active = [&](int t, int it) {
-            const int blk = (p.kv_order == 0) ? it : n_it - 1 - it;
-            return blk < n_tile[t];
-        };
-        auto issue_qk = [&](int t, int st) {
-#pragma unroll
-            for (int ks = 0; ks < C::D / C::KSTEP; ++ks) {
-                const int c = (ks * 32) / 128, w = (ks * 32) % 128;
-                const uint64_t da = ptx::make_smem_desc(ptx::smem_u32(sQ + t * C::TILE + c * (128 * 128) + w), 16, 1024);
-                const uint64_t db = ptx::make_smem_desc(ptx::smem_u32(sK + st * C::TILE + c * (128 * 128) + w), 16, 1024);
-                ptx::mma_ss<C::KIND>(tbase + C::TM_S + t * 128, da, db, idesc_qk, ks > 0 ? 1u : 0u);
-            }
-        };
-        auto issue_pv = [&](int t, int st, uint32_t acc) {
-#pragma unroll
-            for (int ks = 0; ks < C::BN / C::KSTEP; ++ks) {
-                const uint32_t ta = tbase + C::TM_S + t * 128 + ks * 8;
-                const uint64_t db = ptx::make_smem_desc(ptx::smem_u32(sV + st * C::TILE + ks * (C::KSTEP * 128)),
-                                                        C::BN * 128, 1024);
-                ptx::mma_ts<C::KIND>(tbase + C::TM_O + t * 128, ta, db, idesc_pv, acc);
-                acc = 1;
-            }
-        };
-        int cnt[2] = {0, 0};   // blocks of tile t whose P.V has been issued
-        // prologue: S_t(0)
-        for (int t = 0; t < 2; ++t)
-            if (n_tile[t] > 0) ptx::mbar_wait(q_full + t, 0);
-        ptx::mbar_wait(k_full + 0, 0);
-        ptx::tc_fence_after();
-        for (int t = 0; t < 2; ++t)
-            if (active(t, 0)) {
-                issue_qk(t, 0);
-                ptx::tc_commit(s_full + t);
-            }
-        ptx::tc_commit(k_empty + 0);
-        for (int it = 0; it < n_it; ++it) {
+        constexpr uint32_t desc_hi = ptx::smem_desc_hi(1024);
+        const uint32_t q_lo = ptx::smem_desc_lo(ptx::smem_u32(sQ + t * C::TILE), 16);
+        const uint32_t k_lo = ptx::smem_desc_lo(ptx::smem_u32(sK), 16);
+        const uint32_t v_lo = ptx::smem_desc_lo(ptx::smem_u32(sV), C::BN * 128);
+        const uint32_t tS = tbase + C::TM_S + t * 128, tO = tbase + C::TM_O + t * 128;
+        const int first = (p.kv_order == 0) ? 0 : n_it - n_t;
+        const int n_other = n_tile[t ^ 1];
+        const int first_other = (p.kv_order == 0) ? 0 : n_it - n_other;
+        uint64_t* const sf = s_full + 4 * t;
+        uint64_t* const pf = p_full + 4 * t;
+
+        // S_t[:, NG g .. NG (g+1)) = Q_t K[NG g .. NG (g+1), :]^T on ring iteration it
+        auto qk_group = [&](const int g, const int it) {
             const int st = it % C::NS;
-            const uint32_t ph = (it / C::NS) & 1;
-            const bool more = it + 1 < n_it;
-            const int st1 = (it + 1) % C::NS;
-            const uint32_t ph1 = ((it + 1) / C::NS) & 1;
-            bool v_waited = false, k_waited = false;
-            for (int t = 0; t < 2; ++t) {
-                if (active(t, it)) {
-                    ptx::mbar_wait(p_full + t, cnt[t] & 1);
-                    if (!v_waited) {
-                        ptx::mbar_wait(v_full + st, ph);
-                        v_waited = true;
-                    }
-                    ptx::tc_fence_after();
-                    issue_pv(t, st, cnt[t] > 0 ? 1u : 0u);
-                    ++cnt[t];
-                    if (cnt[t] == n_tile[t]) ptx::tc_commit(o_done + t);
+            if (g == 0) {
+                ptx::mbar_wait(k_full + st, (it / C::NS) & 1);
+                ptx::tc_fence_after();
+            }
+            if (leader) {
+                const uint32_t b0 = k_lo + st * (C::TILE >> 4) + g * ((NG * 128) >> 4);
+#pragma unroll
+                for (int ks = 0; ks < C::D / C::KSTEP; ++ks) {
+                    const uint32_t o = (((ks * 32) / 128) * (128 * 128) + (ks * 32) % 128) >> 4;
+                    ptx::mma_ss<C::KIND>(tS + g * NG, ptx::pack2u(q_lo + o, desc_hi), ptx::pack2u(b0 + o, desc_hi),
+                                         idesc_qk, ks > 0 ? 1u : 0u);
                 }
-                if (t == 1) ptx::tc_commit(v_empty + st);
-                if (more && active(t, it + 1)) {
-                    if (!k_waited) {
-                        ptx::mbar_wait(k_full + st1, ph1);
-                        ptx::tc_fence_after();
-                        k_waited = true;
-                    }
-                    issue_qk(t, st1);
-                    ptx::tc_commit(s_full + t);
+                ptx::tc_commit(sf + g);
+                if (g == QKG - 1) {
+                    ptx::tc_commit(k_empty + st);
+                    if (it < first_other || it >= first_other + n_other) ptx::tc_commit(k_empty + st);
                 }
-                if (t == 1 && more) ptx::tc_commit(k_empty + st1);
+            }
+        };
+        // O_t += P_t[:, 32q .. 32q+32) V[32q .. 32q+32, :]
+        auto pv_group = [&](const int q, const int it, const uint32_t acc0, const bool last_of_tile) {
+            const int st = it % C::NS;
+            if (q == 0) {
+                ptx::mbar_wait(v_full + st, (it / C::NS) & 1);
+                ptx::tc_fence_after();
+            }
+            if (leader) {
+                const uint32_t b0 = v_lo + st * (C::TILE >> 4) + q * ((32 * 128) >> 4);
+                uint32_t acc = acc0;
+#pragma unroll
+                for (int ks = 0; ks < 32 / C::KSTEP; ++ks) {
+                    ptx::mma_ts<C::KIND>(tO, tS + q * 32 + ks * 8, ptx::pack2u(b0 + ks * ((C::KSTEP * 128) >> 4), desc_hi),
+                                         idesc_pv, acc);
+                    acc = 1;
+                }
+                if (last_of_tile) ptx::tc_commit(o_done + t);
+                if (q == 3) {
+                    ptx::tc_commit(v_empty + st);
+                    if (it < first_other || it >= first_other + n_other) ptx::tc_commit(v_empty + st);
+                }
+            }
+        };
+
+        ptx::mbar_wait(q_full + t, 0);
+        ptx::tc_fence_after();
+#pragma unroll
+        for (int g = 0; g < QKG; ++g) qk_group(g, first);
+        for (int c = 0; c < n_t; ++c) {
+            const int it = c + first;
+            const bool has_next = c + 1 < n_t;
+#pragma unroll
+            for (int q = 0; q < 4; ++q) {
+                ptx::mbar_wait(pf + q, c & 1);
+                ptx::tc_fence_after();
+                pv_group(q, it, (c > 0 || q > 0) ? 1u : 0u, !has_next && q == 3);
+                if (has_next && (q + 1) % QPG == 0) qk_group(q / QPG, it + 1);
             }
         }
     }

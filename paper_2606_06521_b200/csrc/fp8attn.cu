@@ -4,6 +4,7 @@
 // point that computes returns FP8ATTN_E_DEVICE.
 #include <cmath>
 #include <cstdarg>
+#include <cstdlib>
 #include <cstring>
 #include <mutex>
 
@@ -161,11 +162,11 @@ int dispatch_general(int d, int bn, const CUtensorMap& mq, const CUtensorMap& mk
 }
 
 // ---------------------------------------------------------------------------- prefill kernel launch
-template <int EB, bool FOLD>
-int launch_prefill(const CUtensorMap& mq, const CUtensorMap& mk, const CUtensorMap& mv, const FwdParams& p,
+template <int EB, bool FOLD, int QKG>
+int launch_prefill_g(const CUtensorMap& mq, const CUtensorMap& mk, const CUtensorMap& mv, const FwdParams& p,
                    cudaStream_t st) {
     using C = PrefillCfg<EB>;
-    auto kern = attn_prefill_kernel<EB, FOLD>;
+    auto kern = attn_prefill_kernel<EB, FOLD, QKG>;
     static bool configured = false;
     if (!configured) {
         CU_TRY(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, C::SMEM_BYTES));
@@ -175,6 +176,21 @@ int launch_prefill(const CUtensorMap& mq, const CUtensorMap& mk, const CUtensorM
     kern<<<grid, C::THREADS, C::SMEM_BYTES, st>>>(mq, mk, mv, p);
     CU_TRY(cudaGetLastError());
     return FP8ATTN_OK;
+}
+
+// QK^T issue granularity (1, 2 or 4 groups per block).  FP8ATTN_QKG overrides the default: a tuning knob, the
+// result does not depend on it.
+template <int EB, bool FOLD>
+int launch_prefill(const CUtensorMap& mq, const CUtensorMap& mk, const CUtensorMap& mv, const FwdParams& p,
+                   cudaStream_t st) {
+    static const int qkg = [] {
+        const char* e = getenv("FP8ATTN_QKG");
+        const int v = e ? atoi(e) : 0;
+        return (v == 1 || v == 2 || v == 4) ? v : 2;
+    }();
+    if (qkg == 1) return launch_prefill_g<EB, FOLD, 1>(mq, mk, mv, p, st);
+    if (qkg == 4) return launch_prefill_g<EB, FOLD, 4>(mq, mk, mv, p, st);
+    return launch_prefill_g<EB, FOLD, 2>(mq, mk, mv, p, st);
 }
 
 // S = 2^k with a comfortable exponent: the factor can be folded into the exponent of P exactly
