@@ -11,6 +11,7 @@
 #include "../../include/fp8attn.h"
 #include "attn_general.cuh"
 #include "attn_prefill.cuh"
+#include "attn_decode.cuh"
 #include "debug_gemm.cuh"
 #include "prep.cuh"
 
@@ -178,6 +179,43 @@ int launch_prefill_g(const CUtensorMap& mq, const CUtensorMap& mk, const CUtenso
     return FP8ATTN_OK;
 }
 
+// ---------------------------------------------------------------------------- decode kernel launch
+template <int NVT, bool FOLD>
+int launch_decode_t(const CUtensorMap& mq, const CUtensorMap& mk, const CUtensorMap& mv, const FwdParams& p,
+                    cudaStream_t st) {
+    auto kern = attn_decode_kernel<NVT, FOLD>;
+    static bool configured = false;
+    if (!configured) {
+        CU_TRY(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, DecodeCfg::SMEM_BYTES));
+        configured = true;
+    }
+    const dim3 grid((unsigned)(p.B * p.Hkv), (unsigned)p.num_splits);
+    kern<<<grid, DecodeCfg::THREADS, DecodeCfg::SMEM_BYTES, st>>>(mq, mk, mv, p);
+    CU_TRY(cudaGetLastError());
+    return FP8ATTN_OK;
+}
+template <bool FOLD>
+int launch_decode(int nv, const CUtensorMap& mq, const CUtensorMap& mk, const CUtensorMap& mv, const FwdParams& p,
+                  cudaStream_t st) {
+    if (nv <= 4) return launch_decode_t<4, FOLD>(mq, mk, mv, p, st);
+    if (nv <= 8) return launch_decode_t<8, FOLD>(mq, mk, mv, p, st);
+    return launch_decode_t<16, FOLD>(mq, mk, mv, p, st);
+}
+// Number of KV splits for the decode kernel: enough CTAs to fill 2 x 148 resident slots several times over,
+// with a last wave that is nearly full.
+int decode_auto_splits(long long kv_slabs, int nb) {
+    const long long slots = 2 * 148;
+    int best = 1;
+    for (int ns = 1; ns <= 16 && ns <= nb; ++ns) {
+        const long long ctas = kv_slabs * ns;
+        const long long waves = (ctas + slots - 1) / slots;
+        best = ns;
+        if (ctas >= 4 * slots && (double)ctas / (double)(waves * slots) >= 0.95) break;
+        if (nb / ns < 8) break;      // keep at least 8 blocks per split
+    }
+    return best;
+}
+
 // QK^T issue granularity (1, 2 or 4 groups per block).  FP8ATTN_QKG overrides the default: a tuning knob, the
 // result does not depend on it.
 template <int EB, bool FOLD>
@@ -268,6 +306,12 @@ int fp8attn_fwd(const void* q, const void* k, const void* v, void* o, int B, int
     cudaStream_t st = stats ? reinterpret_cast<cudaStream_t>(stats->stream) : nullptr;
     const int nb = (Lk + bn - 1) / bn;
     const int n_qtiles = (Lq + BM - 1) / BM;
+    const int want_kernel_early = stats ? stats->kernel : 0;
+    const bool decode_shape = pm == 2 && d == 128 && bn == 128 && (long long)(Hq / Hkv) * Lq <= 16 &&
+                              !(stats && (stats->p_codes || stats->underflow));
+    if (ns == 0 && decode_shape && want_kernel_early != 1 && want_kernel_early != 2) {
+        ns = decode_auto_splits(kv_slabs, nb);
+    }
     if (ns == 0) {
         // automatic: split only decode-shaped calls (a handful of query rows per head) whose query
         // tiles alone cannot fill the GPU.  Splitting changes which P values are cast against the
@@ -369,12 +413,21 @@ int fp8attn_fwd(const void* q, const void* k, const void* v, void* o, int B, int
     const bool prefill_ok = d == 128 && bn == 128 && ns == 1 && npl == 1 && pm != 0 && dt != 3 && !p.p_codes &&
                             !p.underflow;
     if (want_kernel == 2 && !prefill_ok) return FP8ATTN_E_UNSUPPORTED;
-    if (want_kernel == 3) return FP8ATTN_E_UNSUPPORTED;
-    const bool use_prefill = prefill_ok && (want_kernel == 2 || (want_kernel == 0 && Lq > 16));
+    const bool decode_ok = decode_shape && eb == 1 && npl == 1;
+    if (want_kernel == 3 && !decode_ok) return FP8ATTN_E_UNSUPPORTED;
+    const bool use_decode = decode_ok && (want_kernel == 3 || want_kernel == 0);
+    const bool use_prefill = !use_decode && prefill_ok && (want_kernel == 2 || (want_kernel == 0 && Lq > 16));
     int kernel_id = 1;
     const dim3 grid((unsigned)n_qtiles, (unsigned)q_slabs, (unsigned)ns);
     int rc;
-    if (use_prefill) {
+    if (use_decode) {
+        kernel_id = 3;
+        // the G*Lq query rows of one kv head are consecutive rows of q: one 16-row box per CTA
+        CUtensorMap mq16;
+        if (int rc2 = make_map(&mq16, qs, 1, 1, q_slabs * Lq, d, 16)) return rc2;
+        const int nv = (Hq / Hkv) * Lq;
+        rc = is_pow2_scale(S) ? launch_decode<true>(nv, mq16, mk, mv, p, st) : launch_decode<false>(nv, mq16, mk, mv, p, st);
+    } else if (use_prefill) {
         kernel_id = 2;
         const bool fold = is_pow2_scale(S);
         if (eb == 1) rc = fold ? launch_prefill<1, true>(mq, mk, mv, p, st) : launch_prefill<1, false>(mq, mk, mv, p, st);
