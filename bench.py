@@ -52,6 +52,17 @@ def load_peaks():
     return {"hbm_gbs": 6650.0, "bf16_tflops": 1590.0, "bf16_tflops_sustained": 1400.0, "source": "fallback"}
 
 
+def ncu_traffic(workload, kernel):
+    """dram__bytes_read.sum + dram__bytes_write.sum of the dominant kernel, per launch, from the committed
+    `ncu --set full` capture of this workload (profiles/traffic.json; null if none was taken)."""
+    try:
+        t = json.load(open(os.path.join(ROOT, "profiles", "traffic.json")))
+        e = t.get(workload, {})
+        return e.get("dram_bytes_per_launch") if e.get("kernel") == kernel else None
+    except (OSError, ValueError):
+        return None
+
+
 # --------------------------------------------------------------------------- clocks
 class ClockSampler:
     """nvidia-smi clock / throttle-reason samples during the timed region."""
@@ -61,6 +72,18 @@ class ClockSampler:
 
     def __init__(self, index):
         self.index, self.proc, self.lines = index, None, []
+        self.lo = self.hi = None
+
+    def mark_start(self):
+        """Timed region starts: wait for the sampler's first line (nvidia-smi takes a moment to come up)."""
+        t0 = time.time()
+        while self.proc and not self.lines and time.time() - t0 < 3.0:
+            time.sleep(0.01)
+        self.lo = len(self.lines)
+
+    def mark_end(self):
+        time.sleep(0.06)
+        self.hi = len(self.lines)
 
     def __enter__(self):
         try:
@@ -82,7 +105,8 @@ class ClockSampler:
     def summary(self):
         sm, mx, reasons = [], [], set()
         names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
-        for ln in self.lines:
+        lines = self.lines[self.lo:self.hi] if self.lo is not None and self.hi is not None else self.lines
+        for ln in lines:
             f = [x.strip() for x in ln.split(",")]
             if len(f) < 7:
                 continue
@@ -158,19 +182,21 @@ def run_ours(args, rank, world, dev):
     def step():
         return fa.fwd(q, k, v, causal=cfg.causal, S=S, kv_order=order, mode=mode, out=o, **sc)
 
-    for _ in range(max(args.warmup, 3)):
-        r = step()
-    torch.cuda.synchronize()
-    if world > 1:
-        dist.barrier()
-    ev = [torch.cuda.Event(enable_timing=True) for _ in range(args.steps + 1)]
-    torch.cuda.synchronize()
     with ClockSampler(dev.index or 0) as clk:
+        for _ in range(max(args.warmup, 3)):
+            r = step()
+        torch.cuda.synchronize()
+        if world > 1:
+            dist.barrier()
+        ev = [torch.cuda.Event(enable_timing=True) for _ in range(args.steps + 1)]
+        torch.cuda.synchronize()
+        clk.mark_start()
         ev[0].record()
         for i in range(args.steps):
             step()
             ev[i + 1].record()
         torch.cuda.synchronize()
+        clk.mark_end()
     if world > 1:
         dist.barrier()
     per_step = [ev[i].elapsed_time(ev[i + 1]) for i in range(args.steps)]
@@ -224,9 +250,9 @@ def run_ours(args, rank, world, dev):
         roof = {"bound": "hbm", "achieved": amount / (kern_ms * 1e-3), "peak": peaks["hbm_gbs"], "unit": "GB/s",
                 "peak_source": f"{peaks['source']} copy bandwidth"}
     roof["frac"] = roof["achieved"] / roof["peak"]
-    roof["traffic"] = None
     roof["kernel_ms"] = kern_ms
     roof["kernel"] = {1: "attn_general_kernel", 2: "attn_prefill_kernel", 3: "attn_decode_kernel"}.get(r.kernel_id, "?")
+    roof["traffic"] = ncu_traffic(args.workload, roof["kernel"])
     line = {
         "metric": "FP8 attention forward throughput" if bound == "tensor" else "split-KV decode attention bandwidth",
         "value": value, "unit": unit, "n_gpus": world, "steps": args.steps, "warmup": max(args.warmup, 3),
@@ -351,7 +377,7 @@ def run_reference(args):
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
-    ap.add_argument("--steps", type=int, default=20)
+    ap.add_argument("--steps", type=int, default=200)
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--workload", choices=sorted(WORKLOADS), default="cfg3")
     ap.add_argument("--impl", choices=["ours", "reference"], default="ours")
