@@ -11,6 +11,7 @@
 #include "../../include/fp8attn.h"
 #include "attn_general.cuh"
 #include "attn_prefill.cuh"
+#include "attn_prefill64.cuh"
 #include "attn_decode.cuh"
 #include "debug_gemm.cuh"
 #include "prep.cuh"
@@ -168,6 +169,23 @@ int launch_prefill_g(const CUtensorMap& mq, const CUtensorMap& mk, const CUtenso
                    cudaStream_t st) {
     using C = PrefillCfg<EB>;
     auto kern = attn_prefill_kernel<EB, FOLD, QKG>;
+    static bool configured = false;
+    if (!configured) {
+        CU_TRY(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, C::SMEM_BYTES));
+        configured = true;
+    }
+    const dim3 grid((unsigned)((p.Lq + 2 * BM - 1) / (2 * BM)), (unsigned)(p.B * p.Hq));
+    kern<<<grid, C::THREADS, C::SMEM_BYTES, st>>>(mq, mk, mv, p);
+    CU_TRY(cudaGetLastError());
+    return FP8ATTN_OK;
+}
+
+// ---------------------------------------------------------------------------- Bn = 64 prefill kernel launch
+template <int EB, bool FOLD>
+int launch_prefill64(const CUtensorMap& mq, const CUtensorMap& mk, const CUtensorMap& mv, const FwdParams& p,
+                     cudaStream_t st) {
+    using C = Prefill64Cfg<EB>;
+    auto kern = attn_prefill64_kernel<EB, FOLD>;
     static bool configured = false;
     if (!configured) {
         CU_TRY(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, C::SMEM_BYTES));
@@ -410,7 +428,7 @@ int fp8attn_fwd(const void* q, const void* k, const void* v, void* o, int B, int
     // kernel family: the warp-specialised prefill kernel serves d = 128, Bn = 128, one split, BF16 or
     // E4M3 operands, modes 1 and 2, when neither the P dump nor the underflow counters are asked for.
     const int want_kernel = stats ? stats->kernel : 0;
-    const bool prefill_ok = d == 128 && bn == 128 && ns == 1 && npl == 1 && pm != 0 && dt != 3 && !p.p_codes &&
+    const bool prefill_ok = d == 128 && (bn == 128 || bn == 64) && ns == 1 && npl == 1 && pm != 0 && dt != 3 && !p.p_codes &&
                             !p.underflow;
     if (want_kernel == 2 && !prefill_ok) return FP8ATTN_E_UNSUPPORTED;
     const bool decode_ok = decode_shape && eb == 1 && npl == 1;
@@ -430,7 +448,10 @@ int fp8attn_fwd(const void* q, const void* k, const void* v, void* o, int B, int
     } else if (use_prefill) {
         kernel_id = 2;
         const bool fold = is_pow2_scale(S);
-        if (eb == 1) rc = fold ? launch_prefill<1, true>(mq, mk, mv, p, st) : launch_prefill<1, false>(mq, mk, mv, p, st);
+        if (bn == 64) {
+            if (eb == 1) rc = fold ? launch_prefill64<1, true>(mq, mk, mv, p, st) : launch_prefill64<1, false>(mq, mk, mv, p, st);
+            else rc = fold ? launch_prefill64<2, true>(mq, mk, mv, p, st) : launch_prefill64<2, false>(mq, mk, mv, p, st);
+        } else if (eb == 1) rc = fold ? launch_prefill<1, true>(mq, mk, mv, p, st) : launch_prefill<1, false>(mq, mk, mv, p, st);
         else rc = fold ? launch_prefill<2, true>(mq, mk, mv, p, st) : launch_prefill<2, false>(mq, mk, mv, p, st);
     } else if (npl == 3)
         rc = (pm == 0) ? dispatch_general<2, 3, 0>(d, bn, mq, mk, mv, p, grid, st)

@@ -21,19 +21,21 @@ SHAPES = [
     (1, 3, 1, 1, 517, False),           # one query row (forced onto this kernel)
     (1, 2, 1, 257, 700, True),          # second pair has one row
     (1, 1, 1, 1280, 1280, True),        # ring wrap-around: 10 blocks > NS
+    (1, 2, 1, 384, 1700, True),         # Lk - Lq not a multiple of the block: two partly masked blocks per tile
 ]
 
 
 @pytest.mark.parametrize("shape", SHAPES)
 @pytest.mark.parametrize("kind,mode", [("bf16", 1), ("e4m3", 2)])
 @pytest.mark.parametrize("order,S", [(0, 16.0), (1, 256.0), (1, 448.0), (0, 1.0)])
-def test_prefill_kernel_matches_oracle(shape, kind, mode, order, S):
+@pytest.mark.parametrize("bn", [128, 64])
+def test_prefill_kernel_matches_oracle(shape, kind, mode, order, S, bn):
     B, Hq, Hkv, Lq, Lk, causal = shape
     q, k, v = W.sink_qkv(B, Hq, Hkv, Lq, Lk, 128, 6.0, seed=5)
     case = P.make_case(q, k, v, kind)
-    r = P.run_gpu(case, causal=causal, S=S, order=order, mode=mode, block_n=128, num_splits=1, kernel=2,
+    r = P.run_gpu(case, causal=causal, S=S, order=order, mode=mode, block_n=bn, num_splits=1, kernel=2,
                   underflow=False)
-    assert r.kernel_id == 2 and r.block_n == 128 and r.num_splits == 1
+    assert r.kernel_id == 2 and r.block_n == bn and r.num_splits == 1
     ref = P.run_oracle(case, r, causal=causal, S=S, order=order, mode=mode)
     P.check(case, r, ref, mode=mode, label=f"prefill {shape} {kind} S={S} order={order}",
             check_mse=(Lq * Lk > 20000))
@@ -43,7 +45,7 @@ def test_prefill_kernel_matches_oracle(shape, kind, mode, order, S):
         assert np.all(np.isneginf(r.row_max.cpu().numpy()[:, :, :Lq - Lk]))
         assert np.all(r.row_sum.cpu().numpy()[:, :, :Lq - Lk] == 0)
     # the general kernel on the same call: same semantics, same Bn
-    g = P.run_gpu(case, causal=causal, S=S, order=order, mode=mode, block_n=128, num_splits=1, kernel=1)
+    g = P.run_gpu(case, causal=causal, S=S, order=order, mode=mode, block_n=bn, num_splits=1, kernel=1)
     assert g.kernel_id == 1
     og, op = g.o.cpu().numpy().astype(np.float64), r.o.cpu().numpy().astype(np.float64)
     assert P.rel_l2(op, og) <= (2e-4 if mode == 1 else 1e-3)
