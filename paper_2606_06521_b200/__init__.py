@@ -3,7 +3,7 @@
 The CUDA library is loaded lazily (first use of `fp8attn`), so that importing
 `paper_2606_06521_b200.workloads` never touches it.
 """
-__all__ = ["fp8attn", "workloads"]
+__all__ = ["fp8attn", "workloads", "sharding"]
 
 
 def __getattr__(name):
