@@ -34,6 +34,7 @@ struct FwdParams {
     int B, Hq, Hkv, Lq, Lk, causal, kv_order, n_sink, num_splits, nb;
     int q_slabs, kv_slabs;   // B*Hq, B*Hkv: plane stride of the staged operands, in slabs
     float S, sm_scale;
+    int alternate;           // attn_prefill3: the two tiles of a CTA take turns on the MUFU pipe (tuning knob)
 };
 
 // MODE 0: no cast (P kept as three BF16 planes h+m+l = FP32 P exactly)

@@ -1,0 +1,430 @@
+// attn_prefill4.cuh -- prefill kernel, fourth structure: every softmax warp works on BOTH query tiles.
+//
+// Same arithmetic as attn_prefill.cuh (Alg. 1: exact running max after every block, l from
+// the FP32 pre-cast P, cvt.rn.satfinite.e4m3x2.f32 of P*S, epilogue O / (S l)); d = 128, Bn = 128, two
+// 128-row query tiles per CTA.  Measured on B200: a successful mbarrier wait costs ~130 cycles, so the chain
+// "last P quarter -> issuer notices -> P.V + QK^T -> commit -> softmax warp notices -> load S" is 600-900
+// cycles during which the softmax warp of that tile has nothing to do.  Here the two softmax warps of a
+// scheduler do not own one tile each; they own one HALF of the key columns of both tiles:
+//   warp (wq, half): rows 32 wq .. 32 wq + 31 of tile 0 and of tile 1, key columns 64 half .. 64 half + 63
+// and alternate between the tiles: while a warp is in the exp pass of tile 1, the tensor pipe turns tile 0
+// around, and vice versa, so the chain is hidden and both warps of a scheduler are in an exp pass together
+// (two warps keep the MUFU pipe ~90 % busy, one alone cannot).  The price is one exchange per block: the two
+// warps of a row pair swap their 64-column maxima through shared memory and a 64-thread named barrier.
+// Each warp loads its 64 logits of a row once, keeps them in registers through max and exp, and sums its
+// own columns (both warps use the same running max, so the partial row sums just add in the epilogue).
+// O <- alpha O (Alg. 1 line 10, first half) is done by a correction warpgroup per tile.
+// Roles (640 threads, register budgets moved with setmaxnreg):
+//   warps 0-3 / 4-7    softmax, column half 0 / 1 (one query row per lane = TMEM lane, both tiles)
+//   warps 8-11 / 12-15 correction of tile 0 / 1
+//   warps 16, 17       tcgen05.mma issuers of tile 0 / 1;  warp 18 TMA producer;  19 idle
+// TMEM (512 columns): S0 [0,128) S1 [128,256) O0 [256,384) O1 [384,512); P over the head of each S quarter.
+#pragma once
+#include "attn_prefill3.cuh"
+
+namespace fp8attn {
+
+#ifdef FP8ATTN_TRACE
+// development build: per-CTA stamps (globaltimer ns) of thread 0: entry, set-up done, first S seen, loop done,
+// O written; plus the SM id
+__device__ long long g_trace4[4096 * 8];
+__device__ __forceinline__ long long gtime() {
+    long long t;
+    asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t));
+    return t;
+}
+#define FP8ATTN_STAMP4(k)                                                                              \
+    do {                                                                                               \
+        if (threadIdx.x == 0) {                                                                        \
+            const int cta = blockIdx.y * gridDim.x + blockIdx.x;                                       \
+            if (cta < 4096) g_trace4[cta * 8 + (k)] = gtime();                                         \
+        }                                                                                              \
+    } while (0)
+#else
+#define FP8ATTN_STAMP4(k) do { } while (0)
+#endif
+
+template <int EB>
+struct Prefill4Cfg {
+    using P = PrefillCfg<EB>;
+    static constexpr int THREADS = 640;
+    // q_full[2] k_full/k_empty/v_full/v_empty[NS] s_full[2] p_full[2][2] a_full[2][4] o_ready[2] o_done[2]
+    static constexpr int N_BARS = 2 + 4 * P::NS + 2 + 4 + 8 + 2 + 2;
+    // + alpha[2][128] + mx[2 tiles][2 block parities][2 halves][128 rows]
+    static constexpr int SMEM_BYTES = (2 + 2 * P::NS) * P::TILE + 1024 /*align*/ + N_BARS * 8 + 16 + 2 * 128 * 4 +
+                                      2 * 2 * 2 * 128 * 4;
+    static constexpr int REG_SOFTMAX = 144, REG_CORR = 72, REG_MISC = 40;   // 256 (144 + 72) + 128 * 40 <= 640 * 96
+};
+
+// Per-tile constants and running state of a softmax thread (one row of each tile).
+struct RowState {
+    float m_run, l_run;     // running max (raw logit units); partial row sum of this warp's columns (times S if folded)
+    int jlim;               // last visible key of the row
+    long long warp_vis;     // last key visible to every row of the warp
+    float cl2;              // logit scale * log2(e)
+};
+
+// ---- softmax warp (wq, half): Alg. 1 lines 4-9 and 12 for its rows of both tiles, its 64 key columns ----
+template <int EB, bool FOLD>
+__device__ __forceinline__ void prefill4_softmax(const FwdParams& p, int wq, int half, int lane, uint32_t tbase,
+                                                 uint64_t* s_full, uint64_t* p_full, uint64_t* a_full, float* alpha_s,
+                                                 float* mx, uint64_t* o_done, const int* n_tile, int n_it, int pair,
+                                                 int bh, int kvh, const CUtensorMap* mapO, uint8_t* stage0,
+                                                 uint8_t* stage1) {
+    using C = PrefillCfg<EB>;
+    const uint32_t tlane = tbase + (static_cast<uint32_t>(wq * 32) << 16);
+    const int rl = wq * 32 + lane;              // row within the tile = TMEM lane
+    const int off = p.Lk - p.Lq;
+    const int bar_id = 1 + wq;                  // named barrier of the two warps that share these rows
+
+    float c_nat = p.sm_scale, vs = 1.0f;
+    if constexpr (EB == 1) {
+        c_nat *= p.q_scale[bh] * p.k_scale[kvh];
+        vs = p.v_scale[kvh];
+    }
+    const float cl2 = c_nat * LOG2E;
+    const float log2S = FOLD ? log2f(p.S) : 0.0f;   // exact for S = 2^k
+    const uint64_t cl2_2 = ptx::pack2(cl2, cl2), s_2 = ptx::pack2(p.S, p.S);
+
+    int jlim[2], first[2];
+    long long wvis[2];
+    float m_run[2] = {-INFINITY, -INFINITY}, l_run[2] = {0.0f, 0.0f};
+#pragma unroll
+    for (int t = 0; t < 2; ++t) {
+        const int row0 = (pair * 2 + t) * BM;
+        long long jl = p.causal ? (long long)row0 + rl + off : (long long)p.Lk - 1;
+        if (jl > p.Lk - 1) jl = p.Lk - 1;
+        jlim[t] = (int)jl;
+        wvis[t] = p.causal ? (long long)row0 + wq * 32 + off : (long long)p.Lk - 1;
+        first[t] = (p.kv_order == 0) ? 0 : n_it - n_tile[t];
+    }
+
+#pragma unroll 1
+    for (int it = 0; it < n_it; ++it) {
+#pragma unroll
+        for (int tt = 0; tt < 2; ++tt) {
+            const int t = 1 - tt;               // tile 1 first: under a causal mask it has the extra block
+            const int c = it - first[t];
+            if (c < 0 || c >= n_tile[t]) continue;
+            const int blk = (p.kv_order == 0) ? c : n_tile[t] - 1 - c;
+            const int j0 = blk * 128;
+            const bool mask = (j0 + 127 > wvis[t]) || (j0 + 128 > p.Lk);
+            const uint32_t tS = tlane + C::TM_S + t * 128;
+            // ---- this warp's 64 logits of the row, loaded once ----
+            uint32_t r[64];
+            ptx::mbar_wait(s_full + t, c & 1);
+            ptx::tc_fence_after();
+            if (it == 0) FP8ATTN_STAMP4(2);
+            ptx::tmem_ld_x32(tS + half * 64, r);
+            ptx::tmem_ld_x32(tS + half * 64 + 32, r + 32);
+            ptx::tmem_wait_ld();
+            if (mask) {
+                mask32(r, j0 + half * 64, jlim[t]);
+                mask32(r + 32, j0 + half * 64 + 32, jlim[t]);
+            }
+            // ---- lines 4-6: block max (exchanged with the warp of the other column half), running max ----
+            float mloc = fmaxf(max32(r, -INFINITY), max32(r + 32, -INFINITY));
+            float* mxt = mx + (t * 2 + (c & 1)) * 256;
+            mxt[half * 128 + rl] = mloc;
+            ptx::named_bar_sync(bar_id, 64);
+            mloc = fmaxf(mloc, mxt[(half ^ 1) * 128 + rl]);
+            const float m_new = fmaxf(m_run[t], mloc);
+            const float m_used = (m_new == -INFINITY) ? 0.0f : m_new;
+            const float alpha = ptx::ex2_approx((m_run[t] - m_used) * cl2);   // 0 when m_run = -inf
+            const float negm = fmaf(-m_used, cl2, log2S);
+            const uint64_t negm_2 = ptx::pack2(negm, negm);
+            if (half == 0) {                    // alpha goes to the correction warp of these rows
+                alpha_s[t * 128 + rl] = alpha;
+                __syncwarp();
+                if (lane == 0) ptx::mbar_arrive(a_full + 4 * t + wq);
+            }
+            // ---- lines 7-9: two P quarters ----
+            uint64_t sum_a = ptx::pack2(0.f, 0.f), sum_b = sum_a;
+            p_quarter<EB, FOLD>(r, false, tS, 2 * half, j0, jlim[t], cl2_2, negm_2, s_2, sum_a, sum_b,
+                                p_full + 2 * t + 0, lane);
+            p_quarter<EB, FOLD>(r + 32, false, tS, 2 * half + 1, j0, jlim[t], cl2_2, negm_2, s_2, sum_a, sum_b,
+                                p_full + 2 * t + 1, lane);
+            float sa, sb, sc, sd;
+            ptx::unpack2(sum_a, sa, sb);
+            ptx::unpack2(sum_b, sc, sd);
+            l_run[t] = alpha * l_run[t] + ((sa + sb) + (sc + sd));   // line 8 (this warp's columns)
+            m_run[t] = m_new;
+        }
+    }
+
+    FP8ATTN_STAMP4(3);
+    // ---- line 12: O / (S l), statistics.  Each warp owns 32 rows x 64 output columns of each tile: it scales
+    // them, writes them as two 32-row x 128-byte boxes (128-byte swizzle) into the K / V ring, which no MMA reads
+    // any more once both tiles are done, and stores the boxes with TMA (rows >= Lq are clipped by the map) ----
+#pragma unroll
+    for (int t = 0; t < 2; ++t) {
+        if (n_tile[t] > 0) ptx::mbar_wait(o_done + t, 0);
+    }
+    ptx::tc_fence_after();
+#pragma unroll
+    for (int t = 0; t < 2; ++t) {
+        const int row0 = (pair * 2 + t) * BM;
+        const int qrow = row0 + rl;
+        const long long grow = (long long)bh * p.Lq + qrow;
+        float* mxt = mx + t * 512;
+        ptx::named_bar_sync(bar_id, 64);        // the partner has read the last block maximum
+        mxt[half * 128 + rl] = l_run[t];
+        ptx::named_bar_sync(bar_id, 64);
+        const float l_all = l_run[t] + mxt[(half ^ 1) * 128 + rl];
+        const float l_true = FOLD ? l_all / p.S : l_all;
+        if (qrow < p.Lq && half == 0) {
+            if (p.row_max) p.row_max[grow] = (m_run[t] == -INFINITY) ? -INFINITY : m_run[t] * c_nat;
+            if (p.row_sum) p.row_sum[grow] = l_true;
+        }
+        const float inv = (l_all > 0.0f) ? (FOLD ? vs / l_all : vs / (p.S * l_all)) : 0.0f;
+        if (row0 >= p.Lq) continue;             // no row of this tile exists (warp-uniform)
+        const uint32_t tO = tlane + C::TM_O + t * 128 + half * 64;
+        uint8_t* stage = t ? stage1 : stage0;
+#pragma unroll 1
+        for (int cb = 0; cb < 2; ++cb) {
+            const int ch = half * 2 + cb;       // 32-column chunk of the output row
+            uint32_t v[32];
+            if (n_tile[t] > 0) {
+                ptx::tmem_ld_x32(tO + cb * 32, v);
+                ptx::tmem_wait_ld();
+            } else {
+#pragma unroll
+                for (int e = 0; e < 32; ++e) v[e] = 0u;
+            }
+            uint8_t* box = stage + (ch * 4 + wq) * 4096;
+#pragma unroll
+            for (int j = 0; j < 8; ++j) {
+                const float4 o4 = make_float4(__uint_as_float(v[4 * j]) * inv, __uint_as_float(v[4 * j + 1]) * inv,
+                                              __uint_as_float(v[4 * j + 2]) * inv, __uint_as_float(v[4 * j + 3]) * inv);
+                *reinterpret_cast<float4*>(box + lane * 128 + ((j ^ (lane & 7)) << 4)) = o4;
+            }
+            ptx::fence_proxy_async_smem();
+            __syncwarp();
+            if (lane == 0) ptx::tma_store_3d(mapO, box, ch * 32, row0 + wq * 32, bh);
+        }
+    }
+    if (lane == 0) {
+        ptx::bulk_commit_group();
+        ptx::bulk_wait_group_read0();
+    }
+}
+
+// ---- the kernel ---------------------------------------------------------------------------------
+// grid = (ceil(Lq / 256), B*Hq).  Causal launches the heaviest tile pairs first.
+template <int EB, bool FOLD>
+__global__ void __launch_bounds__(640, 1)
+attn_prefill4_kernel(const __grid_constant__ CUtensorMap mapQ, const __grid_constant__ CUtensorMap mapK,
+                     const __grid_constant__ CUtensorMap mapV, const __grid_constant__ CUtensorMap mapO,
+                     const FwdParams p) {
+    using C = PrefillCfg<EB>;
+    using C4 = Prefill4Cfg<EB>;
+    extern __shared__ uint8_t smem_raw[];
+    uint8_t* smem = reinterpret_cast<uint8_t*>((reinterpret_cast<uintptr_t>(smem_raw) + 1023) & ~uintptr_t(1023));
+    uint8_t* sQ = smem;                           // 2 tiles
+    uint8_t* sK = sQ + 2 * C::TILE;               // NS tiles
+    uint8_t* sV = sK + C::NS * C::TILE;           // NS tiles
+    uint64_t* bars = reinterpret_cast<uint64_t*>(sV + C::NS * C::TILE);
+    uint64_t* q_full = bars;                      // [2]
+    uint64_t* k_full = bars + 2;                  // [NS]
+    uint64_t* k_empty = k_full + C::NS;
+    uint64_t* v_full = k_empty + C::NS;
+    uint64_t* v_empty = v_full + C::NS;
+    uint64_t* s_full = v_empty + C::NS;           // [2 tiles]                   MMA -> softmax
+    uint64_t* p_full = s_full + 2;                // [2 tiles][2 steps]          softmax (8 warps) -> MMA
+    uint64_t* a_full = p_full + 4;                // [2 tiles][4 warps]          softmax warp -> correction warp
+    uint64_t* o_ready = a_full + 8;               // [2]                         correction (4 warps) -> MMA
+    uint64_t* o_done = o_ready + 2;               // [2]
+    uint32_t* tmem_slot = reinterpret_cast<uint32_t*>(o_done + 2);
+    float* alpha_s = reinterpret_cast<float*>(tmem_slot + 4);   // [2 tiles][128 rows]
+    float* mx = alpha_s + 256;                                  // [2 tiles][2 parities][2 halves][128 rows]
+
+    const int tid = threadIdx.x, lane = tid & 31;
+    const int warp = __shfl_sync(0xFFFFFFFFu, tid >> 5, 0);   // provably warp-uniform
+    const int pair = p.causal ? (int)(gridDim.x - 1 - blockIdx.x) : (int)blockIdx.x;
+    const int bh = blockIdx.y;
+    const int b = bh / p.Hq, h = bh % p.Hq;
+    const int kvh = b * p.Hkv + h / (p.Hq / p.Hkv);
+    FP8ATTN_STAMP4(0);
+#ifdef FP8ATTN_TRACE
+    if (tid == 0) {
+        uint32_t smid;
+        asm volatile("mov.u32 %0, %%smid;" : "=r"(smid));
+        const int cta = blockIdx.y * gridDim.x + blockIdx.x;
+        if (cta < 4096) g_trace4[cta * 8 + 7] = smid;
+    }
+#endif
+
+    // visible block count of each tile (bottom-right causal, reading R15)
+    int n_tile[2];
+#pragma unroll
+    for (int t = 0; t < 2; ++t) {
+        const long long r0 = (long long)(pair * 2 + t) * BM;
+        int n = 0;
+        if (r0 < p.Lq) {
+            n = p.nb;
+            if (p.causal) {
+                long long kmax = r0 + (BM - 1) + (p.Lk - p.Lq);
+                if (kmax > p.Lk - 1) kmax = p.Lk - 1;
+                n = kmax < 0 ? 0 : (int)(kmax / C::BN) + 1;
+            }
+        }
+        n_tile[t] = n;
+    }
+    const int n_it = n_tile[0] > n_tile[1] ? n_tile[0] : n_tile[1];
+
+    if (tid == 0) {
+        ptx::prefetch_tmap(&mapQ);
+        ptx::prefetch_tmap(&mapK);
+        ptx::prefetch_tmap(&mapV);
+        ptx::prefetch_tmap(&mapO);
+        for (int i = 0; i < 2; ++i) ptx::mbar_init(q_full + i, 1);
+        for (int i = 0; i < C::NS; ++i) {
+            ptx::mbar_init(k_full + i, 1);
+            ptx::mbar_init(v_full + i, 1);
+            ptx::mbar_init(k_empty + i, 2);   // one arrival per tile
+            ptx::mbar_init(v_empty + i, 2);
+        }
+        for (int i = 0; i < 2; ++i) {
+            ptx::mbar_init(s_full + i, 1);
+            ptx::mbar_init(o_ready + i, 4);
+            ptx::mbar_init(o_done + i, 1);
+        }
+        for (int i = 0; i < 4; ++i) ptx::mbar_init(p_full + i, 8);
+        for (int i = 0; i < 8; ++i) ptx::mbar_init(a_full + i, 1);
+        ptx::fence_mbar_init();
+    }
+    if (warp == 16) {
+        __syncwarp();
+        ptx::tmem_alloc(tmem_slot, 512);
+    }
+    ptx::tc_fence_before();
+    __syncthreads();
+    ptx::tc_fence_after();
+    const uint32_t tbase = *tmem_slot;
+    FP8ATTN_STAMP4(1);
+
+    if (warp < 8) {
+        ptx::setmaxnreg_inc<C4::REG_SOFTMAX>();
+        prefill4_softmax<EB, FOLD>(p, warp & 3, warp >> 2, lane, tbase, s_full, p_full, a_full, alpha_s, mx, o_done,
+                                   n_tile, n_it, pair, bh, kvh, &mapO, sK, sV);
+    } else if (warp < 16) {
+        ptx::setmaxnreg_dec<C4::REG_CORR>();
+        const int t = (warp - 8) >> 2, wq = warp & 3;
+        prefill3_correction(t, wq, lane, tbase, a_full + 4 * t + wq, alpha_s + t * 128 + wq * 32 + lane, o_ready + t,
+                            n_tile[t]);
+    } else {
+        ptx::setmaxnreg_dec<C4::REG_MISC>();
+        if (warp == 18) {
+            // ================= TMA producer =================
+            if (lane == 0 && n_it > 0) {
+                for (int t = 0; t < 2; ++t) {
+                    if (n_tile[t] == 0) continue;
+                    ptx::mbar_arrive_expect_tx(q_full + t, C::TILE);
+                    for (int c = 0; c < C::NCH; ++c)
+                        ptx::tma_load_3d(sQ + t * C::TILE + c * (128 * 128), &mapQ, q_full + t, c * C::CH,
+                                         (pair * 2 + t) * BM, bh);
+                }
+                for (int it = 0; it < n_it; ++it) {
+                    const int blk = (p.kv_order == 0) ? it : n_it - 1 - it;
+                    const int st = it % C::NS;
+                    const uint32_t ph = (it / C::NS) & 1;
+                    ptx::mbar_wait(k_empty + st, ph ^ 1);
+                    ptx::mbar_arrive_expect_tx(k_full + st, C::TILE);
+                    for (int c = 0; c < C::NCH; ++c)
+                        ptx::tma_load_3d(sK + st * C::TILE + c * (128 * 128), &mapK, k_full + st, c * C::CH,
+                                         blk * C::BN, kvh);
+                    ptx::mbar_wait(v_empty + st, ph ^ 1);
+                    ptx::mbar_arrive_expect_tx(v_full + st, C::TILE);
+                    for (int c = 0; c < C::NCH; ++c)
+                        ptx::tma_load_3d(sV + st * C::TILE + c * (128 * 128), &mapV, v_full + st, c * C::CH,
+                                         blk * C::BN, kvh);
+                }
+            }
+        } else if (warp < 18 && n_tile[warp - 16] > 0) {
+            // ================= MMA issuer of tile t = warp - 16 =================
+            // Block c of tile t uses K/V ring iteration it = c + first.  A ring slot is released by two
+            // arrivals, one per tile; on iterations that only one tile uses, that tile arrives twice.
+            const int t = warp - 16;
+            const int n_t = n_tile[t];
+            const bool leader = ptx::elect_one();
+            constexpr uint32_t idesc_qk = ptx::make_idesc(C::FMT, C::FMT, ptx::MAJOR_K, ptx::MAJOR_K, BM, C::BN);
+            constexpr uint32_t idesc_pv = ptx::make_idesc(C::FMT, C::FMT, ptx::MAJOR_K, ptx::MAJOR_MN, BM, C::D);
+            constexpr uint32_t desc_hi = ptx::smem_desc_hi(1024);
+            const uint32_t q_lo = ptx::smem_desc_lo(ptx::smem_u32(sQ + t * C::TILE), 16);
+            const uint32_t k_lo = ptx::smem_desc_lo(ptx::smem_u32(sK), 16);
+            const uint32_t v_lo = ptx::smem_desc_lo(ptx::smem_u32(sV), C::BN * 128);
+            const uint32_t tS = tbase + C::TM_S + t * 128, tO = tbase + C::TM_O + t * 128;
+            const int first = (p.kv_order == 0) ? 0 : n_it - n_t;
+            const int n_other = n_tile[t ^ 1];
+            const int first_other = (p.kv_order == 0) ? 0 : n_it - n_other;
+            uint64_t* const pf = p_full + 2 * t;
+
+            // S_t = Q_t K^T on ring iteration it
+            auto qk_block = [&](const int it) {
+                const int st = it % C::NS;
+                ptx::mbar_wait(k_full + st, (it / C::NS) & 1);
+                ptx::tc_fence_after();
+                if (leader) {
+                    const uint32_t b0 = k_lo + st * (C::TILE >> 4);
+#pragma unroll
+                    for (int ks = 0; ks < C::D / C::KSTEP; ++ks) {
+                        const uint32_t o = (((ks * 32) / 128) * (128 * 128) + (ks * 32) % 128) >> 4;
+                        ptx::mma_ss<C::KIND>(tS, ptx::pack2u(q_lo + o, desc_hi), ptx::pack2u(b0 + o, desc_hi), idesc_qk,
+                                             ks > 0 ? 1u : 0u);
+                    }
+                    ptx::tc_commit(s_full + t);
+                    ptx::tc_commit(k_empty + st);
+                    if (it < first_other || it >= first_other + n_other) ptx::tc_commit(k_empty + st);
+                }
+            };
+            // O_t += P_t[:, 32q .. 32q+32) V[32q .. 32q+32, :]
+            auto pv_quarter = [&](const int q, const int it, const uint32_t acc0) {
+                const int st = it % C::NS;
+                if (leader) {
+                    const uint32_t b0 = v_lo + st * (C::TILE >> 4) + q * ((32 * 128) >> 4);
+                    uint32_t acc = acc0;
+#pragma unroll
+                    for (int ks = 0; ks < 32 / C::KSTEP; ++ks) {
+                        ptx::mma_ts<C::KIND>(tO, tS + q * 32 + ks * 8,
+                                             ptx::pack2u(b0 + ks * ((C::KSTEP * 128) >> 4), desc_hi), idesc_pv, acc);
+                        acc = 1;
+                    }
+                }
+            };
+
+            ptx::mbar_wait(q_full + t, 0);
+            ptx::tc_fence_after();
+            qk_block(first);
+            for (int c = 0; c < n_t; ++c) {
+                const int it = c + first;
+                const int st = it % C::NS;
+                const bool has_next = c + 1 < n_t;
+                ptx::mbar_wait(v_full + st, (it / C::NS) & 1);
+                ptx::mbar_wait(o_ready + t, c & 1);
+                // first quarter of each column half, then the second one (the order the softmax warps write them)
+                ptx::mbar_wait(pf + 0, c & 1);
+                ptx::tc_fence_after();
+                pv_quarter(0, it, c > 0 ? 1u : 0u);
+                pv_quarter(2, it, 1u);
+                ptx::mbar_wait(pf + 1, c & 1);
+                ptx::tc_fence_after();
+                pv_quarter(1, it, 1u);
+                pv_quarter(3, it, 1u);
+                if (leader) {
+                    if (!has_next) ptx::tc_commit(o_done + t);
+                    ptx::tc_commit(v_empty + st);
+                    if (it < first_other || it >= first_other + n_other) ptx::tc_commit(v_empty + st);
+                }
+                if (has_next) qk_block(it + 1);
+            }
+        }
+    }
+
+    FP8ATTN_STAMP4(4);
+    ptx::tc_fence_before();
+    __syncthreads();
+    if (warp == 16) ptx::tmem_dealloc(tbase, 512);
+    FP8ATTN_STAMP4(5);
+}
+
+}  // namespace fp8attn

@@ -12,6 +12,8 @@
 #include "attn_general.cuh"
 #include "attn_prefill.cuh"
 #include "attn_prefill64.cuh"
+#include "attn_prefill3.cuh"
+#include "attn_prefill4.cuh"
 #include "attn_decode.cuh"
 #include "debug_gemm.cuh"
 #include "prep.cuh"
@@ -89,7 +91,9 @@ int make_map(CUtensorMap* m, const void* base, int eb, long long slabs, long lon
     const cuuint64_t gstr[2] = {(cuuint64_t)cols * eb, (cuuint64_t)cols * eb * (cuuint64_t)rows};
     const cuuint32_t box[3] = {(cuuint32_t)(128 / eb), (cuuint32_t)box_rows, 1};
     const cuuint32_t estr[3] = {1, 1, 1};
-    const CUtensorMapDataType dt = (eb == 2) ? CU_TENSOR_MAP_DATA_TYPE_BFLOAT16 : CU_TENSOR_MAP_DATA_TYPE_UINT8;
+    const CUtensorMapDataType dt = (eb == 4)   ? CU_TENSOR_MAP_DATA_TYPE_FLOAT32
+                                   : (eb == 2) ? CU_TENSOR_MAP_DATA_TYPE_BFLOAT16
+                                               : CU_TENSOR_MAP_DATA_TYPE_UINT8;
     CUresult r = fn(m, dt, 3, const_cast<void*>(base), gdim, gstr, box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE,
                     CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
     if (r != CUDA_SUCCESS) {
@@ -180,6 +184,49 @@ int launch_prefill_g(const CUtensorMap& mq, const CUtensorMap& mk, const CUtenso
     return FP8ATTN_OK;
 }
 
+// ---------------------------------------------------------------------------- prefill kernel, third structure
+template <int EB, bool FOLD>
+int launch_prefill3(const CUtensorMap& mq, const CUtensorMap& mk, const CUtensorMap& mv, const FwdParams& p,
+                    cudaStream_t st) {
+    using C = Prefill3Cfg<EB>;
+    auto kern = attn_prefill3_kernel<EB, FOLD>;
+    static const int alternate = [] {
+        const char* e = getenv("FP8ATTN_ALT");
+        return e ? atoi(e) : 1;
+    }();
+    FwdParams pa = p;
+    pa.alternate = alternate;
+    static bool configured = false;
+    if (!configured) {
+        CU_TRY(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, C::SMEM_BYTES));
+        configured = true;
+    }
+    const dim3 grid((unsigned)((p.Lq + 2 * BM - 1) / (2 * BM)), (unsigned)(p.B * p.Hq));
+    kern<<<grid, C::THREADS, C::SMEM_BYTES, st>>>(mq, mk, mv, pa);
+    CU_TRY(cudaGetLastError());
+    return FP8ATTN_OK;
+}
+
+// ---------------------------------------------------------------------------- prefill kernel, fourth structure
+template <int EB, bool FOLD>
+int launch_prefill4(const CUtensorMap& mq, const CUtensorMap& mk, const CUtensorMap& mv, const FwdParams& p,
+                    cudaStream_t st) {
+    using C = Prefill4Cfg<EB>;
+    auto kern = attn_prefill4_kernel<EB, FOLD>;
+    static bool configured = false;
+    if (!configured) {
+        CU_TRY(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, C::SMEM_BYTES));
+        configured = true;
+    }
+    // o as [B*Hq, Lq, d] FP32: boxes of 32 rows x 32 floats, stored by TMA from the epilogue
+    CUtensorMap mo;
+    if (int rc = make_map(&mo, p.o, 4, (long long)p.B * p.Hq, p.Lq, 128, 32)) return rc;
+    const dim3 grid((unsigned)((p.Lq + 2 * BM - 1) / (2 * BM)), (unsigned)(p.B * p.Hq));
+    kern<<<grid, C::THREADS, C::SMEM_BYTES, st>>>(mq, mk, mv, mo, p);
+    CU_TRY(cudaGetLastError());
+    return FP8ATTN_OK;
+}
+
 // ---------------------------------------------------------------------------- Bn = 64 prefill kernel launch
 template <int EB, bool FOLD>
 int launch_prefill64(const CUtensorMap& mq, const CUtensorMap& mk, const CUtensorMap& mv, const FwdParams& p,
@@ -244,6 +291,12 @@ int launch_prefill(const CUtensorMap& mq, const CUtensorMap& mk, const CUtensorM
         const int v = e ? atoi(e) : 0;
         return (v == 1 || v == 2 || v == 4) ? v : 2;
     }();
+    static const int variant = [] {
+        const char* e = getenv("FP8ATTN_PREFILL_V");
+        return e ? atoi(e) : 4;
+    }();
+    if (variant == 4) return launch_prefill4<EB, FOLD>(mq, mk, mv, p, st);
+    if (variant == 3) return launch_prefill3<EB, FOLD>(mq, mk, mv, p, st);
     if (qkg == 1) return launch_prefill_g<EB, FOLD, 1>(mq, mk, mv, p, st);
     if (qkg == 4) return launch_prefill_g<EB, FOLD, 4>(mq, mk, mv, p, st);
     return launch_prefill_g<EB, FOLD, 2>(mq, mk, mv, p, st);
@@ -615,3 +668,15 @@ int fp8attn_debug_gemm(const void* A, const void* Bm, float* D, int N, int K, in
 }
 
 }  // extern "C"
+
+#ifdef FP8ATTN_TRACE
+// development build only: copies the clock64 stamps of attn_prefill3_kernel to the host
+extern "C" __attribute__((visibility("default"))) int fp8attn_debug_trace(long long* out, int n) {
+    if (n > 2 * 80 * 16) n = 2 * 80 * 16;
+    return (int)cudaMemcpyFromSymbol(out, fp8attn::g_trace3, (size_t)n * sizeof(long long));
+}
+extern "C" __attribute__((visibility("default"))) int fp8attn_debug_trace4(long long* out, int n) {
+    if (n > 4096 * 8) n = 4096 * 8;
+    return (int)cudaMemcpyFromSymbol(out, fp8attn::g_trace4, (size_t)n * sizeof(long long));
+}
+#endif
