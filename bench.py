@@ -251,7 +251,7 @@ def run_ours(args, rank, world, dev):
                 "peak_source": f"{peaks['source']} copy bandwidth"}
     roof["frac"] = roof["achieved"] / roof["peak"]
     roof["kernel_ms"] = kern_ms
-    roof["kernel"] = {1: "attn_general_kernel", 2: "attn_prefill_kernel", 3: "attn_decode_kernel"}.get(r.kernel_id, "?")
+    roof["kernel"] = {1: "attn_general_kernel", 2: "attn_prefill4_kernel", 3: "attn_decode_kernel"}.get(r.kernel_id, "?")
     roof["traffic"] = ncu_traffic(args.workload, roof["kernel"])
     line = {
         "metric": "FP8 attention forward throughput" if bound == "tensor" else "split-KV decode attention bandwidth",

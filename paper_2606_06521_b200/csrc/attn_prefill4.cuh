@@ -36,7 +36,7 @@ __device__ __forceinline__ long long gtime() {
 #define FP8ATTN_STAMP4(k)                                                                              \
     do {                                                                                               \
         if (threadIdx.x == 0) {                                                                        \
-            const int cta = blockIdx.y * gridDim.x + blockIdx.x;                                       \
+            const int cta = blockIdx.x;                                                                \
             if (cta < 4096) g_trace4[cta * 8 + (k)] = gtime();                                         \
         }                                                                                              \
     } while (0)
@@ -48,6 +48,7 @@ template <int EB>
 struct Prefill4Cfg {
     using P = PrefillCfg<EB>;
     static constexpr int THREADS = 640;
+    static constexpr int HEAD_GROUP = 16;      // (batch, q head) slabs whose CTAs are launched together
     // q_full[2] k_full/k_empty/v_full/v_empty[NS] s_full[2] p_full[2][2] a_full[2][4] o_ready[2] o_done[2]
     static constexpr int N_BARS = 2 + 4 * P::NS + 2 + 4 + 8 + 2 + 2;
     // + alpha[2][128] + mx[2 tiles][2 block parities][2 halves][128 rows]
@@ -99,6 +100,11 @@ __device__ __forceinline__ void prefill4_softmax(const FwdParams& p, int wq, int
         first[t] = (p.kv_order == 0) ? 0 : n_it - n_tile[t];
     }
 
+    // A successful mbarrier wait takes ~130 cycles to report.  When the next block belongs to the other tile its
+    // S has been ready for a while, so the barrier is probed before the second P quarter of the current block
+    // and the answer is read when the next block starts (probed_tile >= 0: a probe is pending).
+    FP8ATTN_DECL_PROBE_PRED();
+    int probed_tile = -1;
 #pragma unroll 1
     for (int it = 0; it < n_it; ++it) {
 #pragma unroll
@@ -106,13 +112,18 @@ __device__ __forceinline__ void prefill4_softmax(const FwdParams& p, int wq, int
             const int t = 1 - tt;               // tile 1 first: under a causal mask it has the extra block
             const int c = it - first[t];
             if (c < 0 || c >= n_tile[t]) continue;
+            // the block after this one, if it is a block of the other tile
+            const int it_o = it + tt;           // tile 1 -> (it, tile 0);  tile 0 -> (it + 1, tile 1)
+            const int c_o = it_o - first[t ^ 1];
+            const bool probe_next = c_o >= 0 && c_o < n_tile[t ^ 1];
             const int blk = (p.kv_order == 0) ? c : n_tile[t] - 1 - c;
             const int j0 = blk * 128;
             const bool mask = (j0 + 127 > wvis[t]) || (j0 + 128 > p.Lk);
             const uint32_t tS = tlane + C::TM_S + t * 128;
             // ---- this warp's 64 logits of the row, loaded once ----
             uint32_t r[64];
-            ptx::mbar_wait(s_full + t, c & 1);
+            if (probed_tile != t || !ptx::mbar_probe_result()) ptx::mbar_wait(s_full + t, c & 1);
+            probed_tile = -1;
             ptx::tc_fence_after();
             if (it == 0) FP8ATTN_STAMP4(2);
             ptx::tmem_ld_x32(tS + half * 64, r);
@@ -142,6 +153,10 @@ __device__ __forceinline__ void prefill4_softmax(const FwdParams& p, int wq, int
             uint64_t sum_a = ptx::pack2(0.f, 0.f), sum_b = sum_a;
             p_quarter<EB, FOLD>(r, false, tS, 2 * half, j0, jlim[t], cl2_2, negm_2, s_2, sum_a, sum_b,
                                 p_full + 2 * t + 0, lane);
+            if (probe_next) {
+                ptx::mbar_probe(s_full + (t ^ 1), c_o & 1);
+                probed_tile = t ^ 1;
+            }
             p_quarter<EB, FOLD>(r + 32, false, tS, 2 * half + 1, j0, jlim[t], cl2_2, negm_2, s_2, sum_a, sum_b,
                                 p_full + 2 * t + 1, lane);
             float sa, sb, sc, sd;
@@ -210,7 +225,7 @@ __device__ __forceinline__ void prefill4_softmax(const FwdParams& p, int wq, int
 }
 
 // ---- the kernel ---------------------------------------------------------------------------------
-// grid = (ceil(Lq / 256), B*Hq).  Causal launches the heaviest tile pairs first.
+// grid = ceil(Lq / 256) * B*Hq CTAs in one dimension (order: see below).
 template <int EB, bool FOLD>
 __global__ void __launch_bounds__(640, 1)
 attn_prefill4_kernel(const __grid_constant__ CUtensorMap mapQ, const __grid_constant__ CUtensorMap mapK,
@@ -240,8 +255,16 @@ attn_prefill4_kernel(const __grid_constant__ CUtensorMap mapQ, const __grid_cons
 
     const int tid = threadIdx.x, lane = tid & 31;
     const int warp = __shfl_sync(0xFFFFFFFFu, tid >> 5, 0);   // provably warp-uniform
-    const int pair = p.causal ? (int)(gridDim.x - 1 - blockIdx.x) : (int)blockIdx.x;
-    const int bh = blockIdx.y;
+    // 1-D grid, launch order = longest work first within groups of HEAD_GROUP (batch, q head) slabs: a group's
+    // K and V (2 x Lk x 128 B per kv head) stay in L2 while its CTAs run, and only the last group's lightest CTAs
+    // are left for the tail of the kernel.
+    const int n_pairs = (p.Lq + 2 * BM - 1) / (2 * BM), n_heads = p.B * p.Hq;
+    const int grp = (int)blockIdx.x / (C4::HEAD_GROUP * n_pairs);
+    const int rem = (int)blockIdx.x - grp * C4::HEAD_GROUP * n_pairs;
+    const int grp_size = min(C4::HEAD_GROUP, n_heads - grp * C4::HEAD_GROUP);
+    const int pair_idx = rem / grp_size;
+    const int pair = p.causal ? n_pairs - 1 - pair_idx : pair_idx;
+    const int bh = grp * C4::HEAD_GROUP + rem % grp_size;
     const int b = bh / p.Hq, h = bh % p.Hq;
     const int kvh = b * p.Hkv + h / (p.Hq / p.Hkv);
     FP8ATTN_STAMP4(0);
@@ -249,7 +272,7 @@ attn_prefill4_kernel(const __grid_constant__ CUtensorMap mapQ, const __grid_cons
     if (tid == 0) {
         uint32_t smid;
         asm volatile("mov.u32 %0, %%smid;" : "=r"(smid));
-        const int cta = blockIdx.y * gridDim.x + blockIdx.x;
+        const int cta = blockIdx.x;
         if (cta < 4096) g_trace4[cta * 8 + 7] = smid;
     }
 #endif

@@ -221,7 +221,7 @@ int launch_prefill4(const CUtensorMap& mq, const CUtensorMap& mk, const CUtensor
     // o as [B*Hq, Lq, d] FP32: boxes of 32 rows x 32 floats, stored by TMA from the epilogue
     CUtensorMap mo;
     if (int rc = make_map(&mo, p.o, 4, (long long)p.B * p.Hq, p.Lq, 128, 32)) return rc;
-    const dim3 grid((unsigned)((p.Lq + 2 * BM - 1) / (2 * BM)), (unsigned)(p.B * p.Hq));
+    const dim3 grid((unsigned)(((p.Lq + 2 * BM - 1) / (2 * BM)) * (p.B * p.Hq)));
     kern<<<grid, C::THREADS, C::SMEM_BYTES, st>>>(mq, mk, mv, mo, p);
     CU_TRY(cudaGetLastError());
     return FP8ATTN_OK;
