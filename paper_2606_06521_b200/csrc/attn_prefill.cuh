@@ -47,10 +47,39 @@ __device__ __forceinline__ uint32_t e4m3x2_to_bf16x2(uint32_t pair) {
     return r;
 }
 
+// 2^x for a packed pair on the FMA pipe (the MUFU pipe is the busy one in the exp pass): x = n + f with
+// n = round(x) taken from the low mantissa bits of x + 1.5 * 2^23, f in [-0.5, 0.5], a degree-5 polynomial for
+// 2^f (near-minimax, Chebyshev nodes; max relative error 2.3e-7 in FP32 Horner form, the same order as
+// ex2.approx), and n added to the exponent field.  x is clamped at -125 (2^-125 casts to E4M3 zero and adds
+// nothing to a row sum that holds at least one term equal to S).
+__device__ __forceinline__ void exp2_poly2(uint64_t x2, float& r0, float& r1) {
+    constexpr float MAGIC = 12582912.0f;
+    float x0, x1;
+    ptx::unpack2(x2, x0, x1);
+    x0 = fmaxf(x0, -125.0f);
+    x1 = fmaxf(x1, -125.0f);
+    const uint64_t xc = ptx::pack2(x0, x1);
+    const uint64_t t2 = ptx::add2(xc, ptx::pack2(MAGIC, MAGIC));
+    const uint64_t n2 = ptx::add2(t2, ptx::pack2(-MAGIC, -MAGIC));
+    const uint64_t f2 = ptx::fma2(n2, ptx::pack2(-1.0f, -1.0f), xc);
+    uint64_t p2 = ptx::fma2(ptx::pack2(0.00134004f, 0.00134004f), f2, ptx::pack2(0.00967604f, 0.00967604f));
+    p2 = ptx::fma2(p2, f2, ptx::pack2(0.05550327f, 0.05550327f));
+    p2 = ptx::fma2(p2, f2, ptx::pack2(0.24022107f, 0.24022107f));
+    p2 = ptx::fma2(p2, f2, ptx::pack2(0.6931472f, 0.6931472f));
+    p2 = ptx::fma2(p2, f2, ptx::pack2(1.0000001f, 1.0000001f));
+    float p0, p1, t0, t1;
+    ptx::unpack2(p2, p0, p1);
+    ptx::unpack2(t2, t0, t1);
+    r0 = __int_as_float(__float_as_int(p0) + (__float_as_int(t0) << 23));
+    r1 = __int_as_float(__float_as_int(p1) + (__float_as_int(t1) << 23));
+}
+
 // ---- one 32-column chunk of the exp pass (Alg. 1 lines 7-9) -------------------------------------
 // v: raw logits of 32 keys.  Returns P codes / BF16 values in w (P_COLS/4 words) and adds the FP32
 // pre-cast P (times S when the scale is folded into the exponent) to the two packed sums.
-template <int EB, bool FOLD, bool MASK>
+// NPOLY: bit i set = element pair i of the 16 pairs of the chunk takes exp2_poly2 instead of ex2.approx
+// (0: all on the MUFU pipe).
+template <int EB, bool FOLD, bool MASK, int NPOLY = 0>
 __device__ __forceinline__ void exp_chunk(const uint32_t* v, uint32_t* w, int j_first, int jlim, uint64_t cl2_2,
                                           uint64_t negm_2, uint64_t s_2, uint64_t& sum_a, uint64_t& sum_b) {
     float pr[32];
@@ -62,10 +91,14 @@ __device__ __forceinline__ void exp_chunk(const uint32_t* v, uint32_t* w, int j_
             if (j_first + e + 1 > jlim) b = 0xFF800000u;
         }
         const uint64_t x = ptx::fma2(ptx::pack2u(a, b), cl2_2, negm_2);
-        float x0, x1;
-        ptx::unpack2(x, x0, x1);
-        pr[e] = ptx::ex2_approx(x0);
-        pr[e + 1] = ptx::ex2_approx(x1);
+        if ((NPOLY >> (e >> 1)) & 1) {
+            exp2_poly2(x, pr[e], pr[e + 1]);
+        } else {
+            float x0, x1;
+            ptx::unpack2(x, x0, x1);
+            pr[e] = ptx::ex2_approx(x0);
+            pr[e + 1] = ptx::ex2_approx(x1);
+        }
     }
     uint32_t pair[16];
 #pragma unroll

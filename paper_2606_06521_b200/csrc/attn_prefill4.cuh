@@ -49,6 +49,10 @@ struct Prefill4Cfg {
     using P = PrefillCfg<EB>;
     static constexpr int THREADS = 640;
     static constexpr int HEAD_GROUP = 16;      // (batch, q head) slabs whose CTAs are launched together
+#ifndef FP8ATTN_NPOLY
+#define FP8ATTN_NPOLY 0x8080
+#endif
+    static constexpr int NPOLY = FP8ATTN_NPOLY;   // which of the 16 element pairs of a P quarter take the FMA-pipe exp2
     // q_full[2] k_full/k_empty/v_full/v_empty[NS] s_full[2] p_full[2][2] a_full[2][4] o_ready[2] o_done[2]
     static constexpr int N_BARS = 2 + 4 * P::NS + 2 + 4 + 8 + 2 + 2;
     // + alpha[2][128] + mx[2 tiles][2 block parities][2 halves][128 rows]
@@ -73,6 +77,7 @@ __device__ __forceinline__ void prefill4_softmax(const FwdParams& p, int wq, int
                                                  int bh, int kvh, const CUtensorMap* mapO, uint8_t* stage0,
                                                  uint8_t* stage1) {
     using C = PrefillCfg<EB>;
+    using C4 = Prefill4Cfg<EB>;
     const uint32_t tlane = tbase + (static_cast<uint32_t>(wq * 32) << 16);
     const int rl = wq * 32 + lane;              // row within the tile = TMEM lane
     const int off = p.Lk - p.Lq;
@@ -151,14 +156,17 @@ __device__ __forceinline__ void prefill4_softmax(const FwdParams& p, int wq, int
             }
             // ---- lines 7-9: two P quarters ----
             uint64_t sum_a = ptx::pack2(0.f, 0.f), sum_b = sum_a;
-            p_quarter<EB, FOLD>(r, false, tS, 2 * half, j0, jlim[t], cl2_2, negm_2, s_2, sum_a, sum_b,
-                                p_full + 2 * t + 0, lane);
+            // (a masked logit is -inf: exp2_poly2 turns it into 2^-125, which casts to the E4M3 code 0 and is
+            // far below one ulp of a row sum that holds a visible key; rows without any visible key are set to
+            // l = 0 in the epilogue)
+            p_quarter<EB, FOLD, C4::NPOLY>(r, false, tS, 2 * half, j0, jlim[t], cl2_2, negm_2, s_2, sum_a, sum_b,
+                                           p_full + 2 * t + 0, lane);
             if (probe_next) {
                 ptx::mbar_probe(s_full + (t ^ 1), c_o & 1);
                 probed_tile = t ^ 1;
             }
-            p_quarter<EB, FOLD>(r + 32, false, tS, 2 * half + 1, j0, jlim[t], cl2_2, negm_2, s_2, sum_a, sum_b,
-                                p_full + 2 * t + 1, lane);
+            p_quarter<EB, FOLD, C4::NPOLY>(r + 32, false, tS, 2 * half + 1, j0, jlim[t], cl2_2, negm_2, s_2, sum_a,
+                                           sum_b, p_full + 2 * t + 1, lane);
             float sa, sb, sc, sd;
             ptx::unpack2(sum_a, sa, sb);
             ptx::unpack2(sum_b, sc, sd);
@@ -183,9 +191,10 @@ __device__ __forceinline__ void prefill4_softmax(const FwdParams& p, int wq, int
         const long long grow = (long long)bh * p.Lq + qrow;
         float* mxt = mx + t * 512;
         ptx::named_bar_sync(bar_id, 64);        // the partner has read the last block maximum
-        mxt[half * 128 + rl] = l_run[t];
+        const float l_mine = (m_run[t] == -INFINITY) ? 0.0f : l_run[t];   // no visible key: l = 0 exactly
+        mxt[half * 128 + rl] = l_mine;
         ptx::named_bar_sync(bar_id, 64);
-        const float l_all = l_run[t] + mxt[(half ^ 1) * 128 + rl];
+        const float l_all = l_mine + mxt[(half ^ 1) * 128 + rl];
         const float l_true = FOLD ? l_all / p.S : l_all;
         if (qrow < p.Lq && half == 0) {
             if (p.row_max) p.row_max[grow] = (m_run[t] == -INFINITY) ? -INFINITY : m_run[t] * c_nat;
