@@ -52,7 +52,9 @@ struct Prefill4Cfg {
 #ifndef FP8ATTN_NPOLY
 #define FP8ATTN_NPOLY 0x8080
 #endif
-    static constexpr int NPOLY = FP8ATTN_NPOLY;   // which of the 16 element pairs of a P quarter take the FMA-pipe exp2
+    // which of the 16 element pairs of a P quarter take the FMA-pipe exp2.  BF16 operands: none (measured: the
+    // BF16 mode has twice the tensor time and the extra code-to-BF16 conversion, the polynomial costs 6 % there)
+    static constexpr int NPOLY = (EB == 1) ? FP8ATTN_NPOLY : 0;
     // q_full[2] k_full/k_empty/v_full/v_empty[NS] s_full[2] p_full[2][2] a_full[2][4] o_ready[2] o_done[2]
     static constexpr int N_BARS = 2 + 4 * P::NS + 2 + 4 + 8 + 2 + 2;
     // + alpha[2][128] + mx[2 tiles][2 block parities][2 halves][128 rows]

@@ -192,7 +192,7 @@ int launch_prefill3(const CUtensorMap& mq, const CUtensorMap& mk, const CUtensor
     auto kern = attn_prefill3_kernel<EB, FOLD>;
     static const int alternate = [] {
         const char* e = getenv("FP8ATTN_ALT");
-        return e ? atoi(e) : 1;
+        return e ? atoi(e) : 0;
     }();
     FwdParams pa = p;
     pa.alternate = alternate;
@@ -281,8 +281,9 @@ int decode_auto_splits(long long kv_slabs, int nb) {
     return best;
 }
 
-// QK^T issue granularity (1, 2 or 4 groups per block).  FP8ATTN_QKG overrides the default: a tuning knob, the
-// result does not depend on it.
+// Bn = 128 prefill kernels.  FP8ATTN_PREFILL_V selects the structure (4, the default: attn_prefill4.cuh; 3:
+// attn_prefill3.cuh; 1: attn_prefill.cuh, whose QK^T issue granularity FP8ATTN_QKG = 1, 2 or 4 sets).  These are
+// development / cross-check knobs, read once per process: every structure computes the same Alg. 1 values.
 template <int EB, bool FOLD>
 int launch_prefill(const CUtensorMap& mq, const CUtensorMap& mk, const CUtensorMap& mv, const FwdParams& p,
                    cudaStream_t st) {
@@ -567,10 +568,6 @@ int fp8attn_fwd_host(const void* q, const void* k, const void* v, void* o, int B
     void* ws = nullptr;
     if (int rc = host_buf.get(&ws, off, st)) return rc;
     uint8_t* base = static_cast<uint8_t*>(ws);
-    CU_TRY(cudaMemcpyAsync(base + o_q, q, nq * ebq, cudaMemcpyHostToDevice, st));
-    CU_TRY(cudaMemcpyAsync(base + o_k, k, nkv * ebkv, cudaMemcpyHostToDevice, st));
-    CU_TRY(cudaMemcpyAsync(base + o_v, v, nkv * ebkv, cudaMemcpyHostToDevice, st));
-
     fp8attn_stats dstats;
     fp8attn_stats* ds = nullptr;
     if (stats) {
@@ -596,16 +593,102 @@ int fp8attn_fwd_host(const void* q, const void* k, const void* v, void* o, int B
             CU_TRY(cudaMemsetAsync(base + o_pc, 0xFF, (size_t)Lq * Lk, st));
         }
     }
-    if (int rc = fp8attn_fwd(base + o_q, base + o_k, base + o_v, base + o_o, B, Hq, Hkv, Lq, Lk, d, causal, S,
-                             kv_order, mode, ds))
-        return rc;
-    CU_TRY(cudaMemcpyAsync(o, base + o_o, nq * 4, cudaMemcpyDeviceToHost, st));
+    // (batch, kv-head group) slabs are independent and contiguous in q, k, v and o: large
+    // calls are cut into up to 8 pieces so that the upload of piece i+1, the kernel of piece i and the download
+    // of piece i-1 overlap on three streams (PCIe is full duplex).  The P dump and the underflow counters belong
+    // to one whole call and keep the single-piece path.
+    int pieces_b = 1, pieces_h = 1;      // pieces along the batch, and along the kv heads of one batch element
+    const size_t traffic = nq * ebq + 2 * nkv * ebkv + nq * 4;
+    if (traffic >= (size_t(32) << 20) && !(stats && (stats->p_codes || stats->underflow))) {
+        pieces_b = B < 8 ? B : 8;
+        while (pieces_b * pieces_h < 8 && Hkv % (pieces_h * 2) == 0) pieces_h *= 2;
+        if (B >= 8) pieces_h = 1;
+    }
+    const int n_pieces = pieces_b * pieces_h;
+    if (n_pieces == 1) {
+        CU_TRY(cudaMemcpyAsync(base + o_q, q, nq * ebq, cudaMemcpyHostToDevice, st));
+        CU_TRY(cudaMemcpyAsync(base + o_k, k, nkv * ebkv, cudaMemcpyHostToDevice, st));
+        CU_TRY(cudaMemcpyAsync(base + o_v, v, nkv * ebkv, cudaMemcpyHostToDevice, st));
+        if (int rc = fp8attn_fwd(base + o_q, base + o_k, base + o_v, base + o_o, B, Hq, Hkv, Lq, Lk, d, causal, S,
+                                 kv_order, mode, ds))
+            return rc;
+        CU_TRY(cudaMemcpyAsync(o, base + o_o, nq * 4, cudaMemcpyDeviceToHost, st));
+        if (stats) {
+            if (stats->row_max) CU_TRY(cudaMemcpyAsync(stats->row_max, base + o_rm, R * 4, cudaMemcpyDeviceToHost, st));
+            if (stats->row_sum) CU_TRY(cudaMemcpyAsync(stats->row_sum, base + o_rs, R * 4, cudaMemcpyDeviceToHost, st));
+            if (stats->underflow) CU_TRY(cudaMemcpyAsync(stats->underflow, base + o_uf, 16, cudaMemcpyDeviceToHost, st));
+            if (stats->p_codes)
+                CU_TRY(cudaMemcpyAsync(stats->p_codes, base + o_pc, (size_t)Lq * Lk, cudaMemcpyDeviceToHost, st));
+        }
+    } else {
+        static cudaStream_t s_in = nullptr, s_out = nullptr;
+        static cudaEvent_t ev_start = nullptr, ev_in[8], ev_done[8];
+        if (!s_in) {
+            CU_TRY(cudaStreamCreateWithFlags(&s_in, cudaStreamNonBlocking));
+            CU_TRY(cudaStreamCreateWithFlags(&s_out, cudaStreamNonBlocking));
+            CU_TRY(cudaEventCreateWithFlags(&ev_start, cudaEventDisableTiming));
+            for (int i = 0; i < 8; ++i) {
+                CU_TRY(cudaEventCreateWithFlags(&ev_in[i], cudaEventDisableTiming));
+                CU_TRY(cudaEventCreateWithFlags(&ev_done[i], cudaEventDisableTiming));
+            }
+        }
+        CU_TRY(cudaEventRecord(ev_start, st));          // the staging buffer and the scales are ordered on st
+        CU_TRY(cudaStreamWaitEvent(s_in, ev_start, 0));
+        const uint8_t* hq = static_cast<const uint8_t*>(q);
+        const uint8_t* hk = static_cast<const uint8_t*>(k);
+        const uint8_t* hv = static_cast<const uint8_t*>(v);
+        uint8_t* ho = static_cast<uint8_t*>(o);
+        int launches = 0;
+        for (int i = 0; i < n_pieces; ++i) {
+            // piece i: batch elements [b0, b1), kv heads [h0, h0 + hkv_p) of each (one batch element if pieces_h > 1)
+            const int ib = i / pieces_h, ih = i % pieces_h;
+            const int b0 = (int)((long long)B * ib / pieces_b), b1 = (int)((long long)B * (ib + 1) / pieces_b);
+            const int hkv_p = Hkv / pieces_h, hq_p = Hq / pieces_h;
+            const size_t q_slab0 = (size_t)b0 * Hq + (size_t)ih * hq_p, kv_slab0 = (size_t)b0 * Hkv + (size_t)ih * hkv_p;
+            const size_t q_el = q_slab0 * Lq * d, kv_el = kv_slab0 * Lk * d;
+            const size_t q_n = (size_t)(b1 - b0) * hq_p * Lq * d, kv_n = (size_t)(b1 - b0) * hkv_p * Lk * d;
+            CU_TRY(cudaMemcpyAsync(base + o_q + q_el * ebq, hq + q_el * ebq, q_n * ebq, cudaMemcpyHostToDevice, s_in));
+            CU_TRY(cudaMemcpyAsync(base + o_k + kv_el * ebkv, hk + kv_el * ebkv, kv_n * ebkv, cudaMemcpyHostToDevice, s_in));
+            CU_TRY(cudaMemcpyAsync(base + o_v + kv_el * ebkv, hv + kv_el * ebkv, kv_n * ebkv, cudaMemcpyHostToDevice, s_in));
+            CU_TRY(cudaEventRecord(ev_in[i], s_in));
+            CU_TRY(cudaStreamWaitEvent(st, ev_in[i], 0));
+            fp8attn_stats ps;
+            fp8attn_stats* pp = nullptr;
+            if (ds) {
+                ps = dstats;
+                pp = &ps;
+                if (ps.q_scale) ps.q_scale += q_slab0;
+                if (ps.k_scale) ps.k_scale += kv_slab0;
+                if (ps.v_scale) ps.v_scale += kv_slab0;
+                if (ps.row_max) ps.row_max += q_slab0 * Lq;
+                if (ps.row_sum) ps.row_sum += q_slab0 * Lq;
+            }
+            if (int rc = fp8attn_fwd(base + o_q + q_el * ebq, base + o_k + kv_el * ebkv, base + o_v + kv_el * ebkv,
+                                     base + o_o + q_el * 4, b1 - b0, pieces_h > 1 ? hq_p : Hq, pieces_h > 1 ? hkv_p : Hkv,
+                                     Lq, Lk, d, causal, S, kv_order, mode, pp))
+                return rc;
+            if (pp) {
+                launches += ps.n_launches;
+                dstats.block_m_used = ps.block_m_used;
+                dstats.block_n_used = ps.block_n_used;
+                dstats.num_splits_used = ps.num_splits_used;
+                memcpy(dstats.split_bounds, ps.split_bounds, sizeof ps.split_bounds);
+                dstats.kernel_id = ps.kernel_id;
+                dstats.n_launches = launches;
+            }
+            CU_TRY(cudaEventRecord(ev_done[i], st));
+            CU_TRY(cudaStreamWaitEvent(s_out, ev_done[i], 0));
+            CU_TRY(cudaMemcpyAsync(ho + q_el * 4, base + o_o + q_el * 4, q_n * 4, cudaMemcpyDeviceToHost, s_out));
+            if (stats && stats->row_max)
+                CU_TRY(cudaMemcpyAsync(stats->row_max + q_slab0 * Lq, base + o_rm + q_slab0 * Lq * 4,
+                                       (size_t)(b1 - b0) * hq_p * Lq * 4, cudaMemcpyDeviceToHost, s_out));
+            if (stats && stats->row_sum)
+                CU_TRY(cudaMemcpyAsync(stats->row_sum + q_slab0 * Lq, base + o_rs + q_slab0 * Lq * 4,
+                                       (size_t)(b1 - b0) * hq_p * Lq * 4, cudaMemcpyDeviceToHost, s_out));
+        }
+        CU_TRY(cudaStreamSynchronize(s_out));
+    }
     if (stats) {
-        if (stats->row_max) CU_TRY(cudaMemcpyAsync(stats->row_max, base + o_rm, R * 4, cudaMemcpyDeviceToHost, st));
-        if (stats->row_sum) CU_TRY(cudaMemcpyAsync(stats->row_sum, base + o_rs, R * 4, cudaMemcpyDeviceToHost, st));
-        if (stats->underflow) CU_TRY(cudaMemcpyAsync(stats->underflow, base + o_uf, 16, cudaMemcpyDeviceToHost, st));
-        if (stats->p_codes)
-            CU_TRY(cudaMemcpyAsync(stats->p_codes, base + o_pc, (size_t)Lq * Lk, cudaMemcpyDeviceToHost, st));
         stats->block_m_used = dstats.block_m_used;
         stats->block_n_used = dstats.block_n_used;
         stats->num_splits_used = dstats.num_splits_used;

@@ -197,6 +197,26 @@ def test_fwd_host_equals_fwd():
     assert torch.equal(rh.underflow, r.underflow.cpu())
 
 
+@pytest.mark.parametrize("shape", [(2, 8, 2, 4096, 4096), (12, 2, 1, 2048, 2048)])
+def test_fwd_host_pipelined_pieces_equal_fwd(shape):
+    """Calls above 32 MB of host traffic are cut into (batch, kv-head group) pieces whose copies and kernels
+    overlap (csrc/fp8attn.cu, fp8attn_fwd_host): 2 x 2 pieces for the first shape, 8 batch ranges for the second.
+    The pieces are independent, so the result equals the one-call result bit for bit."""
+    f = P.fa()
+    B, Hq, Hkv, Lq, Lk = shape
+    q, k, v = W.sink_qkv(B, Hq, Hkv, Lq, Lk, 128, 7.0, seed=11)
+    case = P.make_case(q, k, v, "e4m3")
+    r = P.run_gpu(case, causal=True, S=256.0, order=1, mode=2, underflow=False)
+    assert r.kernel_id == 2
+    sc = {n: torch.from_numpy(a) for n, a in case.scales.items()}
+    pin = lambda a: torch.from_numpy(a).pin_memory()
+    rh = f.fwd_host(pin(case.q), pin(case.k), pin(case.v), causal=True, S=256.0, kv_order=1, mode=2,
+                    want_stats=True, want_underflow=False, **sc)
+    assert rh.kernel_id == 2 and rh.n_launches > 1
+    assert torch.equal(rh.o, r.o.cpu())
+    assert torch.equal(rh.row_max, r.row_max.cpu()) and torch.equal(rh.row_sum, r.row_sum.cpu())
+
+
 # ------------------------------------------------------------------ BASELINE config 2 (subset)
 @pytest.mark.parametrize("delta", [0.0, 7.0, 10.0, 14.0])
 @pytest.mark.parametrize("S,order", [(1.0, 0), (256.0, 0), (256.0, 1), (448.0, 1)])
