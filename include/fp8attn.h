@@ -129,7 +129,8 @@ FP8ATTN_API int fp8attn_fwd(const void *q, const void *k, const void *v, void *o
  *   on `stats->stream`, runs fp8attn_fwd there, copies o and the requested statistics back and
  *   synchronises that stream before returning, so the outputs are valid on return.
  *   Element sizes follow the dtype bits of `mode`: FP32 4 B, BF16 2 B, E4M3 1 B.
- *   Calls that move 32 MB or more and ask for neither p_codes nor underflow are cut into up to 8
+ *   Calls that move 32 MB or more, ask for neither p_codes nor underflow and do not leave the split
+ *   count of a decode shape ((Hq/Hkv)*Lq <= 16) to the library are cut into up to 8
  *   (batch, kv-head group) pieces -- independent units of the operation -- whose uploads, kernels
  *   and downloads overlap on `stats->stream` and two library-owned copy streams; the results are
  *   those of the single call bit for bit, `n_launches` counts every piece.

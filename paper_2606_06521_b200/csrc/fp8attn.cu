@@ -599,7 +599,10 @@ int fp8attn_fwd_host(const void* q, const void* k, const void* v, void* o, int B
     // to one whole call and keep the single-piece path.
     int pieces_b = 1, pieces_h = 1;      // pieces along the batch, and along the kv heads of one batch element
     const size_t traffic = nq * ebq + 2 * nkv * ebkv + nq * 4;
-    if (traffic >= (size_t(32) << 20) && !(stats && (stats->p_codes || stats->underflow))) {
+    // (the automatic split count of a decode-shaped call depends on B * Hkv: such a call stays whole unless the
+    // caller fixes num_splits, otherwise the pieces would take another split layout than the single call, R14)
+    const bool auto_split = (long long)(Hq / Hkv) * Lq <= 16 && !(stats && stats->num_splits > 0);
+    if (traffic >= (size_t(32) << 20) && !auto_split && !(stats && (stats->p_codes || stats->underflow))) {
         pieces_b = B < 8 ? B : 8;
         while (pieces_b * pieces_h < 8 && Hkv % (pieces_h * 2) == 0) pieces_h *= 2;
         if (B >= 8) pieces_h = 1;
