@@ -86,7 +86,8 @@ typedef struct fp8attn_stats {
     void *stream;              /* cudaStream_t                                                   */
     uint8_t *p_codes;          /* device [Lq, Lk] or NULL: E4M3 code of every P of head
                                   (p_batch, p_head); masked positions hold 0xFF; mode 0 writes
-                                  nothing                                                       */
+                                  nothing.  Served by the general kernel and by the Bn = 128
+                                  prefill kernel (not by the decode and Bn = 64 prefill kernels) */
     int32_t p_batch, p_head;
     /* ---- outputs, device (each may be NULL) ---- */
     float *row_max;            /* [B,Hq,Lq] final running max m (scaled logits, natural log)    */

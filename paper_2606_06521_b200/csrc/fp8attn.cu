@@ -212,11 +212,12 @@ template <int EB, bool FOLD>
 int launch_prefill4(const CUtensorMap& mq, const CUtensorMap& mk, const CUtensorMap& mv, const FwdParams& p,
                     cudaStream_t st) {
     using C = Prefill4Cfg<EB>;
-    auto kern = attn_prefill4_kernel<EB, FOLD>;
-    static bool configured = false;
-    if (!configured) {
+    // the instance with the P dump is a test aid (fp8attn_stats.p_codes): same schedule, codes also to memory
+    auto kern = p.p_codes ? attn_prefill4_kernel<EB, FOLD, true> : attn_prefill4_kernel<EB, FOLD, false>;
+    static bool configured[2] = {false, false};
+    if (!configured[p.p_codes ? 1 : 0]) {
         CU_TRY(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, C::SMEM_BYTES));
-        configured = true;
+        configured[p.p_codes ? 1 : 0] = true;
     }
     // o as [B*Hq, Lq, d] FP32: boxes of 32 rows x 32 floats, stored by TMA from the epilogue
     CUtensorMap mo;
@@ -281,6 +282,13 @@ int decode_auto_splits(long long kv_slabs, int nb) {
     return best;
 }
 
+int prefill_variant() {
+    static const int variant = [] {
+        const char* e = getenv("FP8ATTN_PREFILL_V");
+        return e ? atoi(e) : 4;
+    }();
+    return variant;
+}
 // Bn = 128 prefill kernels.  FP8ATTN_PREFILL_V selects the structure (4, the default: attn_prefill4.cuh; 3:
 // attn_prefill3.cuh; 1: attn_prefill.cuh, whose QK^T issue granularity FP8ATTN_QKG = 1, 2 or 4 sets).  These are
 // development / cross-check knobs, read once per process: every structure computes the same Alg. 1 values.
@@ -292,10 +300,7 @@ int launch_prefill(const CUtensorMap& mq, const CUtensorMap& mk, const CUtensorM
         const int v = e ? atoi(e) : 0;
         return (v == 1 || v == 2 || v == 4) ? v : 2;
     }();
-    static const int variant = [] {
-        const char* e = getenv("FP8ATTN_PREFILL_V");
-        return e ? atoi(e) : 4;
-    }();
+    const int variant = prefill_variant();
     if (variant == 4) return launch_prefill4<EB, FOLD>(mq, mk, mv, p, st);
     if (variant == 3) return launch_prefill3<EB, FOLD>(mq, mk, mv, p, st);
     if (qkg == 1) return launch_prefill_g<EB, FOLD, 1>(mq, mk, mv, p, st);
@@ -482,7 +487,8 @@ int fp8attn_fwd(const void* q, const void* k, const void* v, void* o, int B, int
     // kernel family: the warp-specialised prefill kernel serves d = 128, Bn = 128, one split, BF16 or
     // E4M3 operands, modes 1 and 2, when neither the P dump nor the underflow counters are asked for.
     const int want_kernel = stats ? stats->kernel : 0;
-    const bool prefill_ok = d == 128 && (bn == 128 || bn == 64) && ns == 1 && npl == 1 && pm != 0 && dt != 3 && !p.p_codes &&
+    const bool prefill_ok = d == 128 && (bn == 128 || bn == 64) && ns == 1 && npl == 1 && pm != 0 && dt != 3 &&
+                            (!p.p_codes || (bn == 128 && prefill_variant() == 4)) &&
                             !p.underflow;
     if (want_kernel == 2 && !prefill_ok) return FP8ATTN_E_UNSUPPORTED;
     const bool decode_ok = decode_shape && eb == 1 && npl == 1;

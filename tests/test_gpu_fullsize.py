@@ -124,6 +124,23 @@ def test_cfg3_full_size_sampled_heads():
                                    block_n=r.block_n, rows=rows, **kw)
         compare_head(cfg, r, ref, b, h, rows, 2, f"cfg3 head {(b, h)}")
         assert ref.uf_other_blocks == 0           # Thm 4 on the oracle side at this size
+    # the P codes of one head at full size, written by the dump instance of the same kernel (same schedule),
+    # on 192 sampled rows against the oracle: >= 99.9 % identical, never more than one code step apart
+    b, h = heads[1]
+    rd = f.fwd(q, k, v, causal=True, S=256.0, kv_order=f.ORDER_REVERSE, mode=f.MODE_FP8, dump_head=(b, h), **sc)
+    torch.cuda.synchronize()
+    assert rd.kernel_id == 2 and torch.equal(rd.o, r.o)
+    qo, ko, vo, dt, kw = head_case(cfg, "e4m3", host, q, k, v, sc, b, h)
+    rows = rows_of_head(cfg.Lq, 192, seed=7)
+    ref = oracle.attention_fwd(qo, ko, vo, causal=True, S=256.0, kv_order=1, mode=2, in_dtype=dt, block_n=r.block_n,
+                               rows=rows, want_codes=True, **kw)
+    g = rd.p_codes[torch.from_numpy(rows).to(rd.p_codes.device)].cpu().numpy()
+    vis = ref.p_codes != 0xFF
+    assert np.array_equal(g == 0xFF, ~vis)
+    match = float(np.mean(g[vis] == ref.p_codes[vis]))
+    assert match >= P.CODE_MATCH[2], match
+    assert np.abs(g[vis].astype(np.int32) - ref.p_codes[vis].astype(np.int32)).max() <= 1
+    print(f"cfg3 full size, head {(b, h)}: P code match {match:.6f} over {int(vis.sum())} visible elements")
 
 
 # ------------------------------------------------------------------ config 4

@@ -55,6 +55,37 @@ def test_prefill_kernel_matches_oracle(shape, kind, mode, order, S, bn):
     assert torch.allclose(g.row_sum, r.row_sum, rtol=2e-6, atol=0)
 
 
+@pytest.mark.parametrize("shape", [(1, 2, 1, 600, 1000, False), (2, 4, 2, 130, 130, True), (1, 2, 1, 384, 1700, True),
+                                   (1, 1, 1, 1280, 1280, True)])
+@pytest.mark.parametrize("kind,mode", [("bf16", 1), ("e4m3", 2)])
+@pytest.mark.parametrize("order,S", [(1, 256.0), (0, 1.0), (0, 448.0)])
+def test_prefill_kernel_p_codes_match_oracle(shape, kind, mode, order, S):
+    """The E4M3 code of every visible P of one head, written by the throughput kernel itself (its dump
+    instance: same schedule, FMA-pipe exp2 for 2 of 16 element pairs included), against the oracle's codes:
+    identical for >= 99.99 % (isolation) / 99.9 % (FP8 mode) of the visible elements and never more than one
+    code step apart (north_star)."""
+    B, Hq, Hkv, Lq, Lk, causal = shape
+    q, k, v = W.sink_qkv(B, Hq, Hkv, Lq, Lk, 128, 7.0, seed=9)
+    case = P.make_case(q, k, v, kind)
+    b, h = B - 1, Hq - 1
+    r = P.run_gpu(case, causal=causal, S=S, order=order, mode=mode, block_n=128, num_splits=1, kernel=2,
+                  underflow=False, dump_head=(b, h))
+    assert r.kernel_id == 2 and r.p_codes is not None
+    rows = (b * Hq + h) * Lq + np.arange(Lq)
+    ref = P.run_oracle(case, r, causal=causal, S=S, order=order, mode=mode, rows=rows, want_codes=True)
+    g = r.p_codes.cpu().numpy()
+    vis = ref.p_codes != 0xFF
+    assert np.array_equal(g == 0xFF, ~vis), "mask pattern of the P dump differs"
+    match = float(np.mean(g[vis] == ref.p_codes[vis]))
+    assert match >= P.CODE_MATCH[mode], match
+    step = np.abs(g[vis].astype(np.int32) - ref.p_codes[vis].astype(np.int32))
+    assert step.max(initial=0) <= 1
+    # the dump instance and the plain instance compute the same output
+    r0 = P.run_gpu(case, causal=causal, S=S, order=order, mode=mode, block_n=128, num_splits=1, kernel=2,
+                   underflow=False)
+    assert torch.equal(r0.o, r.o)
+
+
 def test_prefill_is_the_default_for_prefill_shapes():
     q, k, v = W.sink_qkv(1, 2, 2, 256, 256, 128, 7.0, seed=1)
     case = P.make_case(q, k, v, "e4m3")
