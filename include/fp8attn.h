@@ -86,8 +86,10 @@ typedef struct fp8attn_stats {
     void *stream;              /* cudaStream_t                                                   */
     uint8_t *p_codes;          /* device [Lq, Lk] or NULL: E4M3 code of every P of head
                                   (p_batch, p_head); masked positions hold 0xFF; mode 0 writes
-                                  nothing.  Served by the general kernel and by the Bn = 128
-                                  prefill kernel (not by the decode and Bn = 64 prefill kernels) */
+                                  nothing.  p_codes and underflow are served by the general
+                                  kernel (the automatic choice when either is asked for) and, on
+                                  request (kernel = 2), by the statistics instance of the Bn = 128
+                                  prefill kernel; not by the decode and Bn = 64 prefill kernels  */
     int32_t p_batch, p_head;
     /* ---- outputs, device (each may be NULL) ---- */
     float *row_max;            /* [B,Hq,Lq] final running max m (scaled logits, natural log)    */

@@ -98,19 +98,22 @@ __device__ __forceinline__ void load_block(SoftmaxState& s, uint32_t tS, uint64_
 }
 
 // One P quarter: exp / sum / cast (exp_chunk), P over the head of its S quarter, hand-off to the issuer.
-// DUMP: the E4M3 codes of the visible keys also go to dump_row (row of the P dump of fp8attn_stats; BF16 mode
-// recovers the code from its exact BF16 value: times 2^-120, shifted right by 4).
-template <int EB, bool FOLD, int NPOLY = 0, bool DUMP = false>
+// AUX (statistics instance): the E4M3 codes of the visible keys also go to dump_row (row of the P dump of
+// fp8attn_stats) and the zero codes among the visible non-sink keys are counted into *uf (Prop. 1,
+// PAPER.md:147-155).  BF16 mode recovers a code from its exact BF16 value: times 2^-120, shifted right by 4.
+template <int EB, bool FOLD, int NPOLY = 0, bool AUX = false>
 __device__ __forceinline__ void p_quarter(const uint32_t* v, bool mask, uint32_t tS, int quarter, int j0, int jlim,
                                           uint64_t cl2_2, uint64_t negm_2, uint64_t s_2, uint64_t& sum_a,
-                                          uint64_t& sum_b, uint64_t* bar, int lane, uint8_t* dump_row = nullptr) {
+                                          uint64_t& sum_b, uint64_t* bar, int lane, uint8_t* dump_row = nullptr,
+                                          uint32_t* uf = nullptr, int n_sink = 0) {
     using C = PrefillCfg<EB>;
     uint32_t w[C::P_COLS / 4];
     if (mask) exp_chunk<EB, FOLD, true>(v, w, j0 + quarter * 32, jlim, cl2_2, negm_2, s_2, sum_a, sum_b);
     else exp_chunk<EB, FOLD, false, NPOLY>(v, w, j0 + quarter * 32, jlim, cl2_2, negm_2, s_2, sum_a, sum_b);
-    if constexpr (DUMP) {
-        if (dump_row != nullptr) {
+    if constexpr (AUX) {
+        if (dump_row != nullptr || uf != nullptr) {
             const int jq = j0 + quarter * 32;
+            uint32_t zeros = 0;
 #pragma unroll
             for (int e = 0; e < 32; ++e) {
                 uint32_t code;
@@ -121,8 +124,11 @@ __device__ __forceinline__ void p_quarter(const uint32_t* v, bool mask, uint32_t
                     asm("mul.rn.bf16x2 %0, %1, %2;" : "=r"(back) : "r"(w[e >> 1]), "r"(0x03800380u));   // 2^-120
                     code = (back >> (16 * (e & 1) + 4)) & 0xFFu;
                 }
-                if (jq + e <= jlim) dump_row[jq + e] = (uint8_t)code;
+                const bool vis = jq + e <= jlim;
+                if (vis && dump_row != nullptr) dump_row[jq + e] = (uint8_t)code;
+                if (vis && jq + e >= n_sink && code == 0) ++zeros;
             }
+            if (uf != nullptr) *uf += zeros;
         }
     }
     if constexpr (EB == 1) ptx::tmem_st_x8(tS + quarter * 32, w);

@@ -72,7 +72,7 @@ struct RowState {
 };
 
 // ---- softmax warp (wq, half): Alg. 1 lines 4-9 and 12 for its rows of both tiles, its 64 key columns ----
-template <int EB, bool FOLD, bool DUMP>
+template <int EB, bool FOLD, bool AUX>
 __device__ __forceinline__ void prefill4_softmax(const FwdParams& p, int wq, int half, int lane, uint32_t tbase,
                                                  uint64_t* s_full, uint64_t* p_full, uint64_t* a_full, float* alpha_s,
                                                  float* mx, uint64_t* o_done, const int* n_tile, int n_it, int pair,
@@ -95,7 +95,8 @@ __device__ __forceinline__ void prefill4_softmax(const FwdParams& p, int wq, int
     const uint64_t cl2_2 = ptx::pack2(cl2, cl2), s_2 = ptx::pack2(p.S, p.S);
 
     int jlim[2], first[2];
-    uint8_t* dump_row[2];     // DUMP: this row of the P dump (fp8attn_stats.p_codes), else null
+    uint8_t* dump_row[2];     // AUX: this row of the P dump (fp8attn_stats.p_codes), else null
+    uint32_t uf_sink = 0, uf_other = 0;   // AUX: zero codes among visible non-sink keys (sink block / other blocks)
     long long wvis[2];
     float m_run[2] = {-INFINITY, -INFINITY}, l_run[2] = {0.0f, 0.0f};
 #pragma unroll
@@ -106,7 +107,7 @@ __device__ __forceinline__ void prefill4_softmax(const FwdParams& p, int wq, int
         jlim[t] = (int)jl;
         wvis[t] = p.causal ? (long long)row0 + wq * 32 + off : (long long)p.Lk - 1;
         first[t] = (p.kv_order == 0) ? 0 : n_it - n_tile[t];
-        dump_row[t] = (DUMP && p.p_codes != nullptr && bh == p.p_bh && row0 + rl < p.Lq)
+        dump_row[t] = (AUX && p.p_codes != nullptr && bh == p.p_bh && row0 + rl < p.Lq)
                           ? p.p_codes + (size_t)(row0 + rl) * p.Lk
                           : nullptr;
     }
@@ -165,14 +166,19 @@ __device__ __forceinline__ void prefill4_softmax(const FwdParams& p, int wq, int
             // (a masked logit is -inf: exp2_poly2 turns it into 2^-125, which casts to the E4M3 code 0 and is
             // far below one ulp of a row sum that holds a visible key; rows without any visible key are set to
             // l = 0 in the epilogue)
-            p_quarter<EB, FOLD, C4::NPOLY, DUMP>(r, false, tS, 2 * half, j0, jlim[t], cl2_2, negm_2, s_2, sum_a, sum_b,
-                                                 p_full + 2 * t + 0, lane, dump_row[t]);
+            // AUX: the counter this block adds to (blocks that hold a sink key / all others); rows >= Lq do not
+            // exist and are not counted
+            uint32_t* const uf = (AUX && p.underflow != nullptr && (pair * 2 + t) * BM + rl < p.Lq)
+                                     ? (j0 < p.n_sink ? &uf_sink : &uf_other)
+                                     : nullptr;
+            p_quarter<EB, FOLD, C4::NPOLY, AUX>(r, false, tS, 2 * half, j0, jlim[t], cl2_2, negm_2, s_2, sum_a, sum_b,
+                                                p_full + 2 * t + 0, lane, dump_row[t], uf, p.n_sink);
             if (probe_next) {
                 ptx::mbar_probe(s_full + (t ^ 1), c_o & 1);
                 probed_tile = t ^ 1;
             }
-            p_quarter<EB, FOLD, C4::NPOLY, DUMP>(r + 32, false, tS, 2 * half + 1, j0, jlim[t], cl2_2, negm_2, s_2, sum_a,
-                                                 sum_b, p_full + 2 * t + 1, lane, dump_row[t]);
+            p_quarter<EB, FOLD, C4::NPOLY, AUX>(r + 32, false, tS, 2 * half + 1, j0, jlim[t], cl2_2, negm_2, s_2, sum_a,
+                                                sum_b, p_full + 2 * t + 1, lane, dump_row[t], uf, p.n_sink);
             float sa, sb, sc, sd;
             ptx::unpack2(sum_a, sa, sb);
             ptx::unpack2(sum_b, sc, sd);
@@ -182,6 +188,15 @@ __device__ __forceinline__ void prefill4_softmax(const FwdParams& p, int wq, int
     }
 
     FP8ATTN_STAMP4(3);
+    if constexpr (AUX) {
+        if (p.underflow != nullptr) {       // one atomic per warp and counter (ballot / popc style reduction)
+            const uint32_t a = __reduce_add_sync(0xFFFFFFFFu, uf_sink), b2 = __reduce_add_sync(0xFFFFFFFFu, uf_other);
+            if (lane == 0) {
+                if (a) atomicAdd(p.underflow + 0, (unsigned long long)a);
+                if (b2) atomicAdd(p.underflow + 1, (unsigned long long)b2);
+            }
+        }
+    }
     // ---- line 12: O / (S l), statistics.  Each warp owns 32 rows x 64 output columns of each tile: it scales
     // them, writes them as two 32-row x 128-byte boxes (128-byte swizzle) into the K / V ring, which no MMA reads
     // any more once both tiles are done, and stores the boxes with TMA (rows >= Lq are clipped by the map) ----
@@ -241,7 +256,7 @@ __device__ __forceinline__ void prefill4_softmax(const FwdParams& p, int wq, int
 
 // ---- the kernel ---------------------------------------------------------------------------------
 // grid = ceil(Lq / 256) * B*Hq CTAs in one dimension (order: see below).
-template <int EB, bool FOLD, bool DUMP = false>
+template <int EB, bool FOLD, bool AUX = false>
 __global__ void __launch_bounds__(640, 1)
 attn_prefill4_kernel(const __grid_constant__ CUtensorMap mapQ, const __grid_constant__ CUtensorMap mapK,
                      const __grid_constant__ CUtensorMap mapV, const __grid_constant__ CUtensorMap mapO,
@@ -343,7 +358,7 @@ attn_prefill4_kernel(const __grid_constant__ CUtensorMap mapQ, const __grid_cons
 
     if (warp < 8) {
         ptx::setmaxnreg_inc<C4::REG_SOFTMAX>();
-        prefill4_softmax<EB, FOLD, DUMP>(p, warp & 3, warp >> 2, lane, tbase, s_full, p_full, a_full, alpha_s, mx, o_done,
+        prefill4_softmax<EB, FOLD, AUX>(p, warp & 3, warp >> 2, lane, tbase, s_full, p_full, a_full, alpha_s, mx, o_done,
                                    n_tile, n_it, pair, bh, kvh, &mapO, sK, sV);
     } else if (warp < 16) {
         ptx::setmaxnreg_dec<C4::REG_CORR>();

@@ -212,12 +212,14 @@ template <int EB, bool FOLD>
 int launch_prefill4(const CUtensorMap& mq, const CUtensorMap& mk, const CUtensorMap& mv, const FwdParams& p,
                     cudaStream_t st) {
     using C = Prefill4Cfg<EB>;
-    // the instance with the P dump is a test aid (fp8attn_stats.p_codes): same schedule, codes also to memory
-    auto kern = p.p_codes ? attn_prefill4_kernel<EB, FOLD, true> : attn_prefill4_kernel<EB, FOLD, false>;
+    // the statistics instance (P dump, underflow counters of fp8attn_stats) has the same schedule; the plain
+    // instance carries none of that code
+    const int aux = (p.p_codes || p.underflow) ? 1 : 0;
+    auto kern = aux ? attn_prefill4_kernel<EB, FOLD, true> : attn_prefill4_kernel<EB, FOLD, false>;
     static bool configured[2] = {false, false};
-    if (!configured[p.p_codes ? 1 : 0]) {
+    if (!configured[aux]) {
         CU_TRY(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, C::SMEM_BYTES));
-        configured[p.p_codes ? 1 : 0] = true;
+        configured[aux] = true;
     }
     // o as [B*Hq, Lq, d] FP32: boxes of 32 rows x 32 floats, stored by TMA from the epilogue
     CUtensorMap mo;
@@ -488,13 +490,15 @@ int fp8attn_fwd(const void* q, const void* k, const void* v, void* o, int B, int
     // E4M3 operands, modes 1 and 2, when neither the P dump nor the underflow counters are asked for.
     const int want_kernel = stats ? stats->kernel : 0;
     const bool prefill_ok = d == 128 && (bn == 128 || bn == 64) && ns == 1 && npl == 1 && pm != 0 && dt != 3 &&
-                            (!p.p_codes || (bn == 128 && prefill_variant() == 4)) &&
-                            !p.underflow;
+                            ((!p.p_codes && !p.underflow) || (bn == 128 && prefill_variant() == 4));
     if (want_kernel == 2 && !prefill_ok) return FP8ATTN_E_UNSUPPORTED;
     const bool decode_ok = decode_shape && eb == 1 && npl == 1;
     if (want_kernel == 3 && !decode_ok) return FP8ATTN_E_UNSUPPORTED;
     const bool use_decode = decode_ok && (want_kernel == 3 || want_kernel == 0);
-    const bool use_prefill = !use_decode && prefill_ok && (want_kernel == 2 || (want_kernel == 0 && Lq > 16));
+    // (automatic selection keeps calls that ask for the P dump or the underflow counters on the general kernel;
+    // the statistics instance of the prefill kernel serves them on request, stats->kernel = 2)
+    const bool use_prefill = !use_decode && prefill_ok &&
+                             (want_kernel == 2 || (want_kernel == 0 && Lq > 16 && !p.p_codes && !p.underflow));
     int kernel_id = 1;
     const dim3 grid((unsigned)n_qtiles, (unsigned)q_slabs, (unsigned)ns);
     int rc;

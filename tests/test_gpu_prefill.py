@@ -60,8 +60,9 @@ def test_prefill_kernel_matches_oracle(shape, kind, mode, order, S, bn):
 @pytest.mark.parametrize("kind,mode", [("bf16", 1), ("e4m3", 2)])
 @pytest.mark.parametrize("order,S", [(1, 256.0), (0, 1.0), (0, 448.0)])
 def test_prefill_kernel_p_codes_match_oracle(shape, kind, mode, order, S):
-    """The E4M3 code of every visible P of one head, written by the throughput kernel itself (its dump
-    instance: same schedule, FMA-pipe exp2 for 2 of 16 element pairs included), against the oracle's codes:
+    """The E4M3 code of every visible P of one head and the underflow counters, written by the throughput kernel
+    itself (its statistics instance: same schedule, FMA-pipe exp2 for 2 of 16 element pairs included), against
+    the oracle's:
     identical for >= 99.99 % (isolation) / 99.9 % (FP8 mode) of the visible elements and never more than one
     code step apart (north_star)."""
     B, Hq, Hkv, Lq, Lk, causal = shape
@@ -69,8 +70,11 @@ def test_prefill_kernel_p_codes_match_oracle(shape, kind, mode, order, S):
     case = P.make_case(q, k, v, kind)
     b, h = B - 1, Hq - 1
     r = P.run_gpu(case, causal=causal, S=S, order=order, mode=mode, block_n=128, num_splits=1, kernel=2,
-                  underflow=False, dump_head=(b, h))
-    assert r.kernel_id == 2 and r.p_codes is not None
+                  underflow=True, dump_head=(b, h))
+    assert r.kernel_id == 2 and r.p_codes is not None and r.underflow is not None
+    # output, row statistics and the two underflow counters (Prop. 1) of the whole call
+    P.check(case, r, P.run_oracle(case, r, causal=causal, S=S, order=order, mode=mode), mode=mode,
+            label=f"prefill statistics instance {shape} {kind} S={S} order={order}", check_mse=False)
     rows = (b * Hq + h) * Lq + np.arange(Lq)
     ref = P.run_oracle(case, r, causal=causal, S=S, order=order, mode=mode, rows=rows, want_codes=True)
     g = r.p_codes.cpu().numpy()
@@ -92,7 +96,9 @@ def test_prefill_is_the_default_for_prefill_shapes():
     r = P.run_gpu(case, causal=True, S=256.0, order=1, mode=2, stats=False)
     assert r.kernel_id == 2 and r.n_launches == 1
     r = P.run_gpu(case, causal=True, S=256.0, order=1, mode=2, stats=True)      # underflow counters wanted
-    assert r.kernel_id == 1
+    assert r.kernel_id == 1                                                      # automatic: general kernel
+    r2 = P.run_gpu(case, causal=True, S=256.0, order=1, mode=2, stats=True, kernel=2)   # on request: this kernel
+    assert r2.kernel_id == 2 and torch.equal(r2.underflow, r.underflow)
     f = P.fa()
     with pytest.raises(f.Fp8AttnError) as e:                                     # FP32 inputs: not this kernel
         P.run_gpu(P.make_case(q, k, v, "f32"), causal=True, S=256.0, order=1, mode=1, kernel=2, stats=False)
