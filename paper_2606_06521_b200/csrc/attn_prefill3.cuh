@@ -111,8 +111,15 @@ __device__ __forceinline__ void p_quarter(const uint32_t* v, bool mask, uint32_t
     if (mask) exp_chunk<EB, FOLD, true>(v, w, j0 + quarter * 32, jlim, cl2_2, negm_2, s_2, sum_a, sum_b);
     else exp_chunk<EB, FOLD, false, NPOLY>(v, w, j0 + quarter * 32, jlim, cl2_2, negm_2, s_2, sum_a, sum_b);
     if constexpr (AUX) {
-        if (dump_row != nullptr || uf != nullptr) {
-            const int jq = j0 + quarter * 32;
+        const int jq = j0 + quarter * 32;
+        if (dump_row == nullptr && uf != nullptr && jq >= n_sink && jq + 31 <= jlim) {
+            // every key of the quarter is visible and none is a sink: count the zero codes a word at a time
+            uint32_t zeros = 0;
+#pragma unroll
+            for (int i = 0; i < C::P_COLS / 4; ++i)
+                zeros += (EB == 1) ? (__popc(__vcmpeq4(w[i], 0u)) >> 3) : (__popc(__vcmpeq2(w[i], 0u)) >> 4);
+            *uf += zeros;
+        } else if (dump_row != nullptr || uf != nullptr) {
             uint32_t zeros = 0;
 #pragma unroll
             for (int e = 0; e < 32; ++e) {
