@@ -636,7 +636,21 @@ int fp8attn_fwd_host(const void* q, const void* k, const void* v, void* o, int B
     } else {
         static cudaStream_t s_in = nullptr, s_out = nullptr;
         static cudaEvent_t ev_start = nullptr, ev_in[8], ev_done[8];
+        static int s_dev = -1;
+        int dev_now = 0;
+        cudaGetDevice(&dev_now);
+        if (s_in && s_dev != dev_now) {      // streams and events belong to the device they were created on
+            cudaStreamDestroy(s_in);
+            cudaStreamDestroy(s_out);
+            cudaEventDestroy(ev_start);
+            for (int i = 0; i < 8; ++i) {
+                cudaEventDestroy(ev_in[i]);
+                cudaEventDestroy(ev_done[i]);
+            }
+            s_in = nullptr;
+        }
         if (!s_in) {
+            s_dev = dev_now;
             CU_TRY(cudaStreamCreateWithFlags(&s_in, cudaStreamNonBlocking));
             CU_TRY(cudaStreamCreateWithFlags(&s_out, cudaStreamNonBlocking));
             CU_TRY(cudaEventCreateWithFlags(&ev_start, cudaEventDisableTiming));
