@@ -439,14 +439,22 @@ int fp8attn_fwd(const void* q, const void* k, const void* v, void* o, int B, int
         float* qsc = reinterpret_cast<float*>(codes + ((nq + 15) / 16) * 16);
         unsigned int* amax = static_cast<unsigned int*>(wa);
         const long long slab = (long long)Lq * d;
-        CU_TRY(cudaMemsetAsync(amax, 0, (size_t)q_slabs * 4, st));
-        unsigned gx = (unsigned)((slab + 255) / 256);
-        if (gx > 64) gx = 64;
-        absmax_kernel<__nv_bfloat16><<<dim3(gx, (unsigned)q_slabs), 256, 0, st>>>(static_cast<const __nv_bfloat16*>(q), amax, slab);
-        quantize_kernel<__nv_bfloat16><<<dim3(gx, (unsigned)q_slabs), 256, 0, st>>>(static_cast<const __nv_bfloat16*>(q), amax, codes, slab);
-        finalize_scale_kernel<<<(unsigned)((q_slabs + 255) / 256), 256, 0, st>>>(amax, qsc, (int)q_slabs);
-        CU_TRY(cudaGetLastError());
-        n_launches += 3;
+        if (slab <= 4096) {
+            // a decode-sized q: one warp per slab does absmax, codes and scale in one launch
+            quantize_small_slabs_kernel<__nv_bfloat16><<<(unsigned)((q_slabs + 3) / 4), 128, 0, st>>>(
+                static_cast<const __nv_bfloat16*>(q), codes, qsc, (int)slab, (int)q_slabs);
+            CU_TRY(cudaGetLastError());
+            n_launches += 1;
+        } else {
+            CU_TRY(cudaMemsetAsync(amax, 0, (size_t)q_slabs * 4, st));
+            unsigned gx = (unsigned)((slab + 255) / 256);
+            if (gx > 64) gx = 64;
+            absmax_kernel<__nv_bfloat16><<<dim3(gx, (unsigned)q_slabs), 256, 0, st>>>(static_cast<const __nv_bfloat16*>(q), amax, slab);
+            quantize_kernel<__nv_bfloat16><<<dim3(gx, (unsigned)q_slabs), 256, 0, st>>>(static_cast<const __nv_bfloat16*>(q), amax, codes, slab);
+            finalize_scale_kernel<<<(unsigned)((q_slabs + 255) / 256), 256, 0, st>>>(amax, qsc, (int)q_slabs);
+            CU_TRY(cudaGetLastError());
+            n_launches += 3;
+        }
         qs = codes;
         q_scale = qsc;
     }

@@ -85,6 +85,29 @@ __global__ void quantize_kernel(const T* __restrict__ x, const unsigned int* __r
     }
 }
 
+// The three steps above in one launch for small slabs (the BF16 q of a decode call: Lq * d elements per slab):
+// one warp per slab, same arithmetic in the same order, so codes and scales are bit-identical.
+template <typename T>
+__global__ void quantize_small_slabs_kernel(const T* __restrict__ x, uint8_t* __restrict__ codes,
+                                            float* __restrict__ scale, int slab_elems, int n_slabs) {
+    const int slab = blockIdx.x * (blockDim.x >> 5) + (threadIdx.x >> 5), lane = threadIdx.x & 31;
+    if (slab >= n_slabs) return;
+    const T* xs = x + (long long)slab * slab_elems;
+    uint8_t* cs = codes + (long long)slab * slab_elems;
+    float m = 0.0f;
+    for (int i = lane; i < slab_elems; i += 32) m = fmaxf(m, fabsf(load_as_f32<T>(xs, i)));
+    for (int o = 16; o > 0; o >>= 1) m = fmaxf(m, __shfl_xor_sync(0xFFFFFFFFu, m, o));
+    const float inv = m > 0.0f ? __fdiv_rn(448.0f, m) : 1.0f;
+    for (int i = lane * 2; i < slab_elems; i += 64) {
+        const float a = __fmul_rn(load_as_f32<T>(xs, i), inv);
+        const float b = (i + 1 < slab_elems) ? __fmul_rn(load_as_f32<T>(xs, i + 1), inv) : 0.0f;
+        const uint32_t pr = ptx::cvt_e4m3x2(a, b);
+        cs[i] = (uint8_t)(pr & 0xFF);
+        if (i + 1 < slab_elems) cs[i + 1] = (uint8_t)(pr >> 8);
+    }
+    if (lane == 0) scale[slab] = m > 0.0f ? __fdiv_rn(m, 448.0f) : 1.0f;
+}
+
 __global__ void finalize_scale_kernel(const unsigned int* __restrict__ amax_bits, float* __restrict__ scale, int n) {
     const int i = blockIdx.x * blockDim.x + threadIdx.x;
     if (i < n) {

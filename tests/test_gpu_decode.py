@@ -50,7 +50,7 @@ def test_decode_is_the_default_for_decode_shapes():
     case = P.make_case(q, k, v, "decode")
     r = P.run_gpu(case, causal=False, S=256.0, order=1, mode=2, stats=False)
     assert r.kernel_id == 3
-    assert r.n_launches == 3 + 1 + (1 if r.num_splits > 1 else 0)     # q quantiser (3), decode, combine
+    assert r.n_launches == 1 + 1 + (1 if r.num_splits > 1 else 0)     # q quantiser (one fused launch), decode, combine
     r = P.run_gpu(case, causal=False, S=256.0, order=1, mode=2, stats=True)          # underflow counters wanted
     assert r.kernel_id == 1
     f = P.fa()
