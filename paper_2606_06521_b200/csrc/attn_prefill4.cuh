@@ -63,14 +63,6 @@ struct Prefill4Cfg {
     static constexpr int REG_SOFTMAX = 144, REG_CORR = 72, REG_MISC = 40;   // 256 (144 + 72) + 128 * 40 <= 640 * 96
 };
 
-// Per-tile constants and running state of a softmax thread (one row of each tile).
-struct RowState {
-    float m_run, l_run;     // running max (raw logit units); partial row sum of this warp's columns (times S if folded)
-    int jlim;               // last visible key of the row
-    long long warp_vis;     // last key visible to every row of the warp
-    float cl2;              // logit scale * log2(e)
-};
-
 // ---- softmax warp (wq, half): Alg. 1 lines 4-9 and 12 for its rows of both tiles, its 64 key columns ----
 template <int EB, bool FOLD, bool AUX>
 __device__ __forceinline__ void prefill4_softmax(const FwdParams& p, int wq, int half, int lane, uint32_t tbase,
@@ -97,7 +89,7 @@ __device__ __forceinline__ void prefill4_softmax(const FwdParams& p, int wq, int
     int jlim[2], first[2];
     uint8_t* dump_row[2];     // AUX: this row of the P dump (fp8attn_stats.p_codes), else null
     uint32_t uf_sink = 0, uf_other = 0;   // AUX: zero codes among visible non-sink keys (sink block / other blocks)
-    long long wvis[2];
+    int mask_from[2];         // blocks whose first key index exceeds this need the mask for some row of the warp
     float m_run[2] = {-INFINITY, -INFINITY}, l_run[2] = {0.0f, 0.0f};
 #pragma unroll
     for (int t = 0; t < 2; ++t) {
@@ -105,7 +97,11 @@ __device__ __forceinline__ void prefill4_softmax(const FwdParams& p, int wq, int
         long long jl = p.causal ? (long long)row0 + rl + off : (long long)p.Lk - 1;
         if (jl > p.Lk - 1) jl = p.Lk - 1;
         jlim[t] = (int)jl;
-        wvis[t] = p.causal ? (long long)row0 + wq * 32 + off : (long long)p.Lk - 1;
+        // a block j0 .. j0 + 127 is unmasked iff every row of the warp sees all of it and it lies inside Lk
+        const long long wvis = p.causal ? (long long)row0 + wq * 32 + off : (long long)p.Lk - 1;
+        long long thr = wvis - 127 < (long long)p.Lk - 128 ? wvis - 127 : (long long)p.Lk - 128;
+        if (thr < -(1ll << 30)) thr = -(1ll << 30);
+        mask_from[t] = (int)thr;
         first[t] = (p.kv_order == 0) ? 0 : n_it - n_tile[t];
         dump_row[t] = (AUX && p.p_codes != nullptr && bh == p.p_bh && row0 + rl < p.Lq)
                           ? p.p_codes + (size_t)(row0 + rl) * p.Lk
@@ -130,7 +126,7 @@ __device__ __forceinline__ void prefill4_softmax(const FwdParams& p, int wq, int
             const bool probe_next = c_o >= 0 && c_o < n_tile[t ^ 1];
             const int blk = (p.kv_order == 0) ? c : n_tile[t] - 1 - c;
             const int j0 = blk * 128;
-            const bool mask = (j0 + 127 > wvis[t]) || (j0 + 128 > p.Lk);
+            const bool mask = j0 > mask_from[t];
             const uint32_t tS = tlane + C::TM_S + t * 128;
             // ---- this warp's 64 logits of the row, loaded once ----
             uint32_t r[64];
