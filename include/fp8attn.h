@@ -17,7 +17,11 @@
  * abort or exit.  No entry point allocates or frees caller-visible memory or synchronises
  * the stream.  Work is enqueued on the CUDA stream given in `stats->stream` (the legacy
  * default stream if `stats` is NULL).  Scratch memory (split-KV partials, BF16 planes of
- * FP32 inputs, quantised q for decode) is owned and cached by the library.
+ * FP32 inputs, quantised q for decode, the staging of fp8attn_fwd_host) is allocated per call,
+ * on that stream, from a library-owned stream-ordered memory pool of the current device and
+ * returned to the pool when the call's work is enqueued: calls on different streams, threads
+ * or devices share no scratch and may run concurrently.  The pool keeps what it has been given
+ * until fp8attn_trim().  Every entry point works on the CURRENT device (cudaSetDevice).
  */
 #ifndef FP8ATTN_H
 #define FP8ATTN_H
@@ -54,9 +58,11 @@ extern "C" {
 #define FP8ATTN_E_MODE         -4   /* unknown mode / dtype / kv_order, or a combination that is
                                        not defined (mode 2 needs E4M3 k,v; modes 0,1 need
                                        FP32/BF16)                                               */
-#define FP8ATTN_E_UNSUPPORTED  -5   /* valid but not built: E4M3 with d != 128, block_n not in
-                                       {0, 64, 128}, FP32 inputs with block_n 128, num_splits
-                                       above FP8ATTN_MAX_SPLITS                                  */
+#define FP8ATTN_E_UNSUPPORTED  -5   /* valid but not built: E4M3 with d != 128 (a 64-byte operand
+                                       row does not fill the 128-byte swizzle row the kernels are
+                                       built on), block_n not in {0, 64, 128}, FP32 inputs with
+                                       block_n 128, num_splits above FP8ATTN_MAX_SPLITS, a kernel
+                                       family that cannot serve the call                        */
 #define FP8ATTN_E_DEVICE       -6   /* current device is not compute capability 10.x             */
 #define FP8ATTN_E_CUDA         -7   /* a CUDA call failed (allocation, tensor map, launch)       */
 #define FP8ATTN_E_STATS        -8   /* stats->struct_size does not match this header             */
@@ -85,11 +91,13 @@ typedef struct fp8attn_stats {
     const float *v_scale;      /* device [B*Hkv]                                                 */
     void *stream;              /* cudaStream_t                                                   */
     uint8_t *p_codes;          /* device [Lq, Lk] or NULL: E4M3 code of every P of head
-                                  (p_batch, p_head); masked positions hold 0xFF; mode 0 writes
-                                  nothing.  p_codes and underflow are served by the general
-                                  kernel (the automatic choice when either is asked for) and, on
-                                  request (kernel = 2), by the statistics instance of the Bn = 128
-                                  prefill kernel; not by the decode and Bn = 64 prefill kernels  */
+                                  (p_batch, p_head); the library fills the buffer with 0xFF first,
+                                  so masked positions hold 0xFF; mode 0 writes nothing.  p_codes and
+                                  underflow are served by every kernel family: the general kernel
+                                  (the automatic choice for prefill shapes that ask for either), the
+                                  statistics instances of the prefill kernels (kernel = 2; same
+                                  schedule as the throughput instance) and of the decode kernel
+                                  (the automatic choice for decode shapes)                        */
     int32_t p_batch, p_head;
     /* ---- outputs, device (each may be NULL) ---- */
     float *row_max;            /* [B,Hq,Lq] final running max m (scaled logits, natural log)    */
@@ -133,7 +141,7 @@ FP8ATTN_API int fp8attn_fwd(const void *q, const void *k, const void *v, void *o
  *   synchronises that stream before returning, so the outputs are valid on return.
  *   Element sizes follow the dtype bits of `mode`: FP32 4 B, BF16 2 B, E4M3 1 B.
  *   Calls that move 32 MB or more, ask for neither p_codes nor underflow and do not leave the split
- *   count of a decode shape ((Hq/Hkv)*Lq <= 16) to the library are cut into up to 8
+ *   count of a decode shape ((Hq/Hkv)*Lq <= 16) to the library are cut into at most 8
  *   (batch, kv-head group) pieces -- independent units of the operation -- whose uploads, kernels
  *   and downloads overlap on `stats->stream` and two library-owned copy streams; the results are
  *   those of the single call bit for bit, `n_launches` counts every piece.
@@ -155,8 +163,9 @@ FP8ATTN_API int fp8attn_quantize_e4m3(const float *x, uint8_t *out_codes, float 
                                       int B, int H, int L, int d, void *stream);
 
 /*
- * fp8attn_debug_gemm -- one-tile tcgen05 GEMM through the same TMA / descriptor / TMEM
- * helpers the attention kernels use; exists so tests can pin those primitives.
+ * fp8attn_debug_gemm -- DIAGNOSTIC, not part of the method: one-tile tcgen05 GEMM through the
+ * same TMA / shared-memory-descriptor / TMEM helpers the attention kernels use, so that a test
+ * can pin those primitives (operand majors, swizzle, A-from-TMEM) against an FP64 product.
  *   D[128,N] (device float32) = A[128,K] . B, FP32 accumulate.
  *   elem_bytes 2 = BF16 (kind::f16), 1 = E4M3 (kind::f8f6f4).
  *   a_in_tmem : 0 = A read from swizzled shared memory, 1 = A staged in TMEM (the P operand path).
@@ -166,6 +175,12 @@ FP8ATTN_API int fp8attn_quantize_e4m3(const float *x, uint8_t *out_codes, float 
  */
 FP8ATTN_API int fp8attn_debug_gemm(const void *A, const void *Bm, float *D, int N, int K,
                                    int elem_bytes, int a_in_tmem, int b_mn_major, void *stream);
+
+/*
+ * fp8attn_trim -- give the scratch memory the library's pool holds on the current device back to
+ * the driver (memory still in use by enqueued work stays until that work has run).
+ */
+FP8ATTN_API int fp8attn_trim(void);
 
 FP8ATTN_API const char *fp8attn_strerror(int code);
 FP8ATTN_API const char *fp8attn_last_cuda_error(void);   /* text of the last CUDA failure */

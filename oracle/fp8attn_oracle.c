@@ -42,13 +42,23 @@
 /* ------------------------------------------------------------------------- */
 
 /* Value of the positive code c = (E<<3)|M, c in 0x00..0x7E.  0x7F is NaN.   */
-static double e4m3_code_value(int c)
+static double e4m3_code_value_eq(int c)
 {
     int E = (c >> 3) & 0xF, M = c & 7;
     if (E == 0)
         return ldexp((double)M / 8.0, -6);       /* Eq. 1: 2^(1-b) * M/8, b = 7 */
     return ldexp(1.0 + (double)M / 8.0, E - 7);  /* Eq. 2: 2^(E-b) * (1+M/8)    */
 }
+
+/* The table of code values {0} U the 126 positive values, filled once from Eq. 1-2 when the
+ * library is loaded; every later use reads the table instead of calling ldexp again. */
+static double g_code_value[0x7F];
+__attribute__((constructor)) static void fill_code_values(void)
+{
+    for (int c = 0; c < 0x7F; ++c)
+        g_code_value[c] = e4m3_code_value_eq(c);
+}
+static double e4m3_code_value(int c) { return g_code_value[c]; }
 
 /* The 126 positive values in code order 0x01..0x7E. */
 ORACLE_API void fp8attn_oracle_e4m3_table(double out[126])
@@ -163,6 +173,7 @@ ORACLE_API void fp8attn_oracle_quantize_e4m3(const float *x, uint8_t *codes, flo
             scale = amax / 448.0f;
         }
         scales[s] = scale;
+#pragma omp parallel for schedule(static)
         for (int64_t e = 0; e < slab_elems; ++e) {
             float y = xs[e] * inv;
             codes[s * slab_elems + e] = fp8attn_oracle_round_e4m3(y);

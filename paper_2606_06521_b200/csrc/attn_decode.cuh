@@ -14,7 +14,7 @@
 // block, l from the FP32 pre-cast P, P*S cast with cvt.rn.satfinite.e4m3x2.f32, O / (S l) at the end (or in the
 // combine kernel when the KV range is split).
 #pragma once
-#include "attn_general.cuh"
+#include "common.cuh"
 
 namespace fp8attn {
 
@@ -37,8 +37,11 @@ __device__ __forceinline__ int float_to_ordered(float f) {
 }
 __device__ __forceinline__ float ordered_to_float(int i) { return __int_as_float(i >= 0 ? i : i ^ 0x7FFFFFFF); }
 
-// NVT: compile-time bound on the query rows handled (4, 8 or 16); nv <= NVT of them are real
-template <int NVT, bool FOLD>
+// NVT: compile-time bound on the query rows handled (4, 8 or 16); nv <= NVT of them are real.
+// AUX: the statistics instance -- same schedule, plus the E4M3 code of every visible P of head (p_batch, p_head)
+// written to fp8attn_stats.p_codes and the zero codes among the visible non-sink keys counted (Prop. 1,
+// PAPER.md:147-155), split into blocks that hold a sink key / all other blocks.
+template <int NVT, bool FOLD, bool AUX = false>
 __global__ void __launch_bounds__(192, 2)
 attn_decode_kernel(const __grid_constant__ CUtensorMap mapQ, const __grid_constant__ CUtensorMap mapK,
                    const __grid_constant__ CUtensorMap mapV, const FwdParams p) {
@@ -195,6 +198,15 @@ attn_decode_kernel(const __grid_constant__ CUtensorMap mapQ, const __grid_consta
             jlim[n] = (n < nv) ? (int)jl : -1;
         }
         const float log2S = FOLD ? log2f(p.S) : 0.0f;
+        // AUX: which query row (if any) belongs to the dumped head; Lq rows of one q head are consecutive n
+        uint32_t uf_sink = 0, uf_other = 0;
+        int dump_n0 = -1;                      // first n of the dumped head, or -1
+        if constexpr (AUX) {
+            if (p.p_codes != nullptr) {
+                const int g = p.p_bh - (b * p.Hq + kvh_in_b * G);
+                if (g >= 0 && g < G) dump_n0 = g * p.Lq;
+            }
+        }
 
         for (int j = 0; j < n_it; ++j) {
             const int blk = (p.kv_order == 0) ? sb0 + j : sb1 - 1 - j;
@@ -251,6 +263,20 @@ attn_decode_kernel(const __grid_constant__ CUtensorMap mapQ, const __grid_consta
                 const uint32_t pair = FOLD ? ptx::cvt_e4m3x2(p0, p1) : ptx::cvt_e4m3x2(p0 * p.S, p1 * p.S);   // line 9
                 prow[n * 128 + ((chunk ^ (n & 7)) << 4)] = (uint8_t)(pair & 0xFFu);
                 prow[(n + 1) * 128 + ((chunk ^ ((n + 1) & 7)) << 4)] = (uint8_t)(pair >> 8);
+                if constexpr (AUX) {
+                    // the same two codes that feed P.V: dump (coalesced over the keys of the block) and count
+#pragma unroll
+                    for (int e = 0; e < 2; ++e) {
+                        const int nn = n + e;
+                        const uint32_t code = e ? (pair >> 8) & 0xFFu : pair & 0xFFu;
+                        const bool vis = key <= jlim[nn];        // jlim = -1 for the padding rows nn >= nv
+                        if (vis && dump_n0 >= 0 && nn >= dump_n0 && nn < dump_n0 + p.Lq)
+                            p.p_codes[(size_t)(nn - dump_n0) * p.Lk + key] = (uint8_t)code;
+                        if (vis && key >= p.n_sink && code == 0u) {
+                            if (blk * C::BN < p.n_sink) ++uf_sink; else ++uf_other;
+                        }
+                    }
+                }
             }
             ptx::fence_proxy_async_smem();
             // ---- line 10, first half: O^T <- O^T * alpha (column n by alpha[n]); needs P.V(j-1) finished ----
@@ -274,6 +300,15 @@ attn_decode_kernel(const __grid_constant__ CUtensorMap mapQ, const __grid_consta
             if (lane == 0) ptx::mbar_arrive(p_full + buf);
         }
 
+        if constexpr (AUX) {
+            if (p.underflow != nullptr) {       // one atomic per warp and counter
+                const uint32_t a = __reduce_add_sync(0xFFFFFFFFu, uf_sink), b2 = __reduce_add_sync(0xFFFFFFFFu, uf_other);
+                if (lane == 0) {
+                    if (a) atomicAdd(p.underflow + 0, (unsigned long long)a);
+                    if (b2) atomicAdd(p.underflow + 1, (unsigned long long)b2);
+                }
+            }
+        }
         // ---- row sums over the 128 keys; line 12 or the partial result of this split ----
 #pragma unroll
         for (int n = 0; n < NVT; ++n) {

@@ -9,33 +9,11 @@
 // Epilogue: O / (S l) (line 12).  The steps of one block are serialised (no overlap): this is
 // the reference-grade kernel that carries every feature (FP32 inputs as three BF16 planes,
 // no-cast mode, P-code dump, underflow counters, split-KV partials); the throughput kernels
-// live in attn_prefill.cuh / attn_decode.cuh.
+// live in attn_prefill.cuh / attn_prefill64.cuh / attn_decode.cuh.
 #pragma once
-#include <cuda_fp16.h>
-#include "ptx.cuh"
+#include "common.cuh"
 
 namespace fp8attn {
-
-constexpr int BM = 128;   // query rows per tile = UMMA M = TMEM lanes
-constexpr float LOG2E = 1.4426950408889634f;
-
-struct FwdParams {
-    float* o;
-    float* row_max;
-    float* row_sum;
-    unsigned long long* underflow;
-    uint8_t* p_codes;
-    int p_bh;
-    const float* q_scale;
-    const float* k_scale;
-    const float* v_scale;
-    float* part_o;    // [ns][rows][d]   unnormalised O of each split
-    float* part_ml;   // [ns][rows][2]   (m in natural-log units of the scaled logit, l)
-    int B, Hq, Hkv, Lq, Lk, causal, kv_order, n_sink, num_splits, nb;
-    int q_slabs, kv_slabs;   // B*Hq, B*Hkv: plane stride of the staged operands, in slabs
-    float S, sm_scale;
-    int alternate;           // attn_prefill3: the two tiles of a CTA take turns on the MUFU pipe (tuning knob)
-};
 
 // MODE 0: no cast (P kept as three BF16 planes h+m+l = FP32 P exactly)
 // MODE 1: isolation (P -> E4M3 -> exact BF16), MODE 2: production FP8 (P E4M3 into kind::f8f6f4)
@@ -80,7 +58,9 @@ attn_general_kernel(const __grid_constant__ CUtensorMap mapQ, const __grid_const
     uint32_t* tmem_slot = reinterpret_cast<uint32_t*>(bars + 6);
 
     const int tid = threadIdx.x, warp = tid >> 5;
-    const int qtile = blockIdx.x, bh = blockIdx.y, split = blockIdx.z;
+    // grid = (query tiles x (batch, q head) slabs, 1, KV splits)
+    const int n_qtiles = (p.Lq + BM - 1) / BM;
+    const int qtile = (int)(blockIdx.x % n_qtiles), bh = (int)(blockIdx.x / n_qtiles), split = blockIdx.z;
     const int b = bh / p.Hq, h = bh % p.Hq;
     const int kvh = b * p.Hkv + h / (p.Hq / p.Hkv);
     const int qrow = qtile * BM + tid;

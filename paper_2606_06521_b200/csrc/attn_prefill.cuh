@@ -1,148 +1,94 @@
-// attn_prefill.cuh -- warp-specialised throughput kernel for Alg. 1, d = 128, Bn = 128.
+// attn_prefill.cuh -- warp-specialised prefill kernel: every softmax warp works on BOTH query tiles.
 //
-// One CTA = two 128-row query tiles (256 consecutive query rows) of one (batch, q head).  Roles:
-//   warps 0-3  softmax of tile 0      warps 4-7  softmax of tile 1   (one query row per thread = TMEM lane)
-//   warps 8, 9 tcgen05.mma issuers of tile 0 / tile 1     warp 10  TMA producer
-// TMEM (512 columns): S0 [0,128) S1 [128,256) O0 [256,384) O1 [384,512); P_t is written over the first
-// head of each 32-column quarter of S_t (8 columns E4M3 / 16 BF16) and read from there as the A operand
-// of O_t += P_t V.  S and P move in quarters: QK^T is issued as four N = 32 MMAs groups, P.V as four K = 32
-// groups, each with its own mbarrier, so the tensor pipe works on quarter q while the softmax warps are
-// still on quarter q+1 and the serial chain exp -> P.V -> QK^T -> max shrinks to one quarter.
-// The tensor pipe executes in issue order: ... PV_0(j), QK_0(j+1), PV_1(j), QK_1(j+1) ..., so while the
-// softmax warps of tile 0 work on S_0(j+1) the tensor core runs tile 1 and vice versa; the two softmax
-// groups share the MUFU pipe, which is the binding unit (16 ex2 / clk / SM against 16384 FP8 FLOP / clk).
-// Semantics are exactly those of attn_general.cuh: the running max is exact after every block (no lazy
-// rescale -- it would change which E4M3 code a P value gets), l is summed from the FP32 pre-cast P
-// (Alg. 1 line 8), P*S is cast with cvt.rn.satfinite.e4m3x2.f32 (line 9), the epilogue divides by S l
-// (line 12).  For S = 2^k the factor is folded into the exponent (exact).
-// No P dump and no underflow counters here: calls that ask for them take the general kernel.
+// Same arithmetic as attn_general.cuh (Alg. 1: exact running max after every block, l from
+// the FP32 pre-cast P, cvt.rn.satfinite.e4m3x2.f32 of P*S, epilogue O / (S l)); d = 128, Bn = 128, two
+// 128-row query tiles per CTA.  Measured on B200: a successful mbarrier wait costs ~130 cycles, so the chain
+// "last P quarter -> issuer notices -> P.V + QK^T -> commit -> softmax warp notices -> load S" is 600-900
+// cycles during which the softmax warp of that tile has nothing to do.  Here the two softmax warps of a
+// scheduler do not own one tile each; they own one HALF of the key columns of both tiles:
+//   warp (wq, half): rows 32 wq .. 32 wq + 31 of tile 0 and of tile 1, key columns 64 half .. 64 half + 63
+// and alternate between the tiles: while a warp is in the exp pass of tile 1, the tensor pipe turns tile 0
+// around, and vice versa, so the chain is hidden and both warps of a scheduler are in an exp pass together
+// (two warps keep the MUFU pipe ~90 % busy, one alone cannot).  The price is one exchange per block: the two
+// warps of a row pair swap their 64-column maxima through shared memory and a 64-thread named barrier.
+// Each warp loads its 64 logits of a row once, keeps them in registers through max and exp, and sums its
+// own columns (both warps use the same running max, so the partial row sums just add in the epilogue).
+// O <- alpha O (Alg. 1 line 10, first half) is done by a correction warpgroup per tile.
+// Roles (640 threads, register budgets moved with setmaxnreg):
+//   warps 0-3 / 4-7    softmax, column half 0 / 1 (one query row per lane = TMEM lane, both tiles)
+//   warps 8-11 / 12-15 correction of tile 0 / 1
+//   warps 16, 17       tcgen05.mma issuers of tile 0 / 1;  warp 18 TMA producer;  19 idle
+// TMEM (512 columns): S0 [0,128) S1 [128,256) O0 [256,384) O1 [384,512); P over the head of each S quarter.
 #pragma once
-#include "attn_general.cuh"
+#include "prefill_common.cuh"
 
 namespace fp8attn {
 
 template <int EB>
-struct PrefillCfg {
-    static constexpr int D = 128, BN = 128;
-    static constexpr int CH = 128 / EB;              // elements per 128-byte swizzle row
-    static constexpr int NCH = D / CH;               // 128-byte chunks per operand row
-    static constexpr int TILE = NCH * 128 * 128;     // bytes of one 128-row operand tile (Q, K_j or V_j)
-    static constexpr int NS = (EB == 1) ? 4 : 2;     // K ring depth = V ring depth
-    static constexpr int KSTEP = 32 / EB;            // contraction elements per MMA
-    static constexpr int P_COLS = BN * EB / 4;       // TMEM columns of P
-    static constexpr int TM_S = 0, TM_O = 256;
-    static constexpr int N_BARS = 2 + 4 * NS + 8 + 8 + 2;
-    static constexpr int SMEM_BYTES = (2 + 2 * NS) * TILE + 1024 /*align*/ + N_BARS * 8 + 16;
-    static constexpr uint32_t KIND = (EB == 1) ? ptx::KIND_F8F6F4 : ptx::KIND_F16;
-    static constexpr uint32_t FMT = (EB == 1) ? ptx::FMT_E4M3 : ptx::FMT_BF16;
-    static constexpr int THREADS = 352;
+struct PrefillKCfg {
+    using P = PrefillCfg<EB>;
+    static constexpr int THREADS = 640;
+    static constexpr int HEAD_GROUP = 16;      // (batch, q head) slabs whose CTAs are launched together
+    // which of the 16 element pairs of a P quarter take the FMA-pipe exp2.  BF16 operands: none (measured: the
+    // BF16 mode has twice the tensor time and the extra code-to-BF16 conversion, the polynomial costs 6 % there)
+    static constexpr int NPOLY = (EB == 1) ? 0x8080 : 0;
+    // q_full[2] k_full/k_empty/v_full/v_empty[NS] s_full[2] p_full[2][2] a_full[2][4] o_ready[2] o_done[2]
+    static constexpr int N_BARS = 2 + 4 * P::NS + 2 + 4 + 8 + 2 + 2;
+    // + alpha[2][128] + mx[2 tiles][2 block parities][2 halves][128 rows]
+    static constexpr int SMEM_BYTES = (2 + 2 * P::NS) * P::TILE + 1024 /*align*/ + N_BARS * 8 + 16 + 2 * 128 * 4 +
+                                      2 * 2 * 2 * 128 * 4;
+    static constexpr int REG_SOFTMAX = 144, REG_CORR = 72, REG_MISC = 40;   // 256 (144 + 72) + 128 * 40 <= 640 * 96
 };
 
-// exact E4M3 pair -> BF16 pair: the code shifted left by 4 is the BF16 bit pattern of value * 2^-120
-// (subnormal codes map to BF16 subnormals), and the packed multiply by 2^120 is exact.
-__device__ __forceinline__ uint32_t e4m3x2_to_bf16x2(uint32_t pair) {
-    const uint32_t spread = ((pair & 0xFF00u) << 12) | ((pair & 0xFFu) << 4);
-    uint32_t r;
-    asm("mul.rn.bf16x2 %0, %1, %2;" : "=r"(r) : "r"(spread), "r"(0x7B807B80u));   // 2^120 in both halves
-    return r;
-}
-
-// 2^x for a packed pair on the FMA pipe (the MUFU pipe is the busy one in the exp pass): x = n + f with
-// n = round(x) taken from the low mantissa bits of x + 1.5 * 2^23, f in [-0.5, 0.5], a degree-5 polynomial for
-// 2^f (near-minimax, Chebyshev nodes; max relative error 2.3e-7 in FP32 Horner form, the same order as
-// ex2.approx), and n added to the exponent field.  x is clamped at -125 (2^-125 casts to E4M3 zero and adds
-// nothing to a row sum that holds at least one term equal to S).
-__device__ __forceinline__ void exp2_poly2(uint64_t x2, float& r0, float& r1) {
-    constexpr float MAGIC = 12582912.0f;
-    float x0, x1;
-    ptx::unpack2(x2, x0, x1);
-    x0 = fmaxf(x0, -125.0f);
-    x1 = fmaxf(x1, -125.0f);
-    const uint64_t xc = ptx::pack2(x0, x1);
-    const uint64_t t2 = ptx::add2(xc, ptx::pack2(MAGIC, MAGIC));
-    const uint64_t n2 = ptx::add2(t2, ptx::pack2(-MAGIC, -MAGIC));
-    const uint64_t f2 = ptx::fma2(n2, ptx::pack2(-1.0f, -1.0f), xc);
-    uint64_t p2 = ptx::fma2(ptx::pack2(0.00134004f, 0.00134004f), f2, ptx::pack2(0.00967604f, 0.00967604f));
-    p2 = ptx::fma2(p2, f2, ptx::pack2(0.05550327f, 0.05550327f));
-    p2 = ptx::fma2(p2, f2, ptx::pack2(0.24022107f, 0.24022107f));
-    p2 = ptx::fma2(p2, f2, ptx::pack2(0.6931472f, 0.6931472f));
-    p2 = ptx::fma2(p2, f2, ptx::pack2(1.0000001f, 1.0000001f));
-    float p0, p1, t0, t1;
-    ptx::unpack2(p2, p0, p1);
-    ptx::unpack2(t2, t0, t1);
-    r0 = __int_as_float(__float_as_int(p0) + (__float_as_int(t0) << 23));
-    r1 = __int_as_float(__float_as_int(p1) + (__float_as_int(t1) << 23));
-}
-
-// ---- one 32-column chunk of the exp pass (Alg. 1 lines 7-9) -------------------------------------
-// v: raw logits of 32 keys.  Returns P codes / BF16 values in w (P_COLS/4 words) and adds the FP32
-// pre-cast P (times S when the scale is folded into the exponent) to the two packed sums.
-// NPOLY: bit i set = element pair i of the 16 pairs of the chunk takes exp2_poly2 instead of ex2.approx
-// (0: all on the MUFU pipe).
-template <int EB, bool FOLD, bool MASK, int NPOLY = 0>
-__device__ __forceinline__ void exp_chunk(const uint32_t* v, uint32_t* w, int j_first, int jlim, uint64_t cl2_2,
-                                          uint64_t negm_2, uint64_t s_2, uint64_t& sum_a, uint64_t& sum_b) {
-    float pr[32];
+// ---- correction warp: O <- alpha O for its 32 rows, once per block ---------------------------------
+__device__ __forceinline__ void prefill_correction(int t, int wq, int lane, uint32_t tbase, uint64_t* a_full_w,
+                                                    const float* alpha_slot, uint64_t* o_ready, int n_t) {
+    const uint32_t tO = tbase + (static_cast<uint32_t>(wq * 32) << 16) + 256 + t * 128;
+    for (int c = 0; c < n_t; ++c) {
+        ptx::mbar_wait(a_full_w, c & 1);
+        const float alpha = *alpha_slot;
+        // alpha(c) is published after S(c) is complete, which implies P.V(c-1) is complete (in-order pipe)
+        if (c > 0 && __any_sync(0xFFFFFFFFu, alpha != 1.0f)) {
+            ptx::tc_fence_after();
+            const uint64_t a2 = ptx::pack2(alpha, alpha);
+            uint32_t va[16], vb[16];
+            ptx::tmem_ld_x16(tO, va);
 #pragma unroll
-    for (int e = 0; e < 32; e += 2) {
-        uint32_t a = v[e], b = v[e + 1];
-        if constexpr (MASK) {
-            if (j_first + e > jlim) a = 0xFF800000u;       // -inf
-            if (j_first + e + 1 > jlim) b = 0xFF800000u;
+            for (int cb = 0; cb < 8; ++cb) {
+                uint32_t* cur = (cb & 1) ? vb : va;
+                uint32_t* nxt = (cb & 1) ? va : vb;
+                ptx::tmem_wait_ld();
+                if (cb < 7) ptx::tmem_ld_x16(tO + (cb + 1) * 16, nxt);
+#pragma unroll
+                for (int e = 0; e < 16; e += 2) {
+                    float y0, y1;
+                    ptx::unpack2(ptx::mul2(ptx::pack2u(cur[e], cur[e + 1]), a2), y0, y1);
+                    cur[e] = __float_as_uint(y0);
+                    cur[e + 1] = __float_as_uint(y1);
+                }
+                ptx::tmem_st_x16(tO + cb * 16, cur);
+            }
+            ptx::tmem_wait_st();
         }
-        const uint64_t x = ptx::fma2(ptx::pack2u(a, b), cl2_2, negm_2);
-        if ((NPOLY >> (e >> 1)) & 1) {
-            exp2_poly2(x, pr[e], pr[e + 1]);
-        } else {
-            float x0, x1;
-            ptx::unpack2(x, x0, x1);
-            pr[e] = ptx::ex2_approx(x0);
-            pr[e + 1] = ptx::ex2_approx(x1);
-        }
-    }
-    uint32_t pair[16];
-#pragma unroll
-    for (int e = 0; e < 32; e += 4) {
-        const uint64_t p0 = ptx::pack2(pr[e], pr[e + 1]), p1 = ptx::pack2(pr[e + 2], pr[e + 3]);
-        sum_a = ptx::add2(sum_a, p0);
-        sum_b = ptx::add2(sum_b, p1);
-    }
-    if constexpr (!FOLD) {
-#pragma unroll
-        for (int e = 0; e < 32; e += 2) {
-            float y0, y1;
-            ptx::unpack2(ptx::mul2(ptx::pack2(pr[e], pr[e + 1]), s_2), y0, y1);
-            pair[e / 2] = ptx::cvt_e4m3x2(y0, y1);
-        }
-    } else {
-#pragma unroll
-        for (int e = 0; e < 32; e += 2) pair[e / 2] = ptx::cvt_e4m3x2(pr[e], pr[e + 1]);
-    }
-    if constexpr (EB == 1) {
-#pragma unroll
-        for (int e = 0; e < 8; ++e) w[e] = pair[2 * e] | (pair[2 * e + 1] << 16);
-    } else {
-#pragma unroll
-        for (int e = 0; e < 16; ++e) w[e] = e4m3x2_to_bf16x2(pair[e]);
+        ptx::tc_fence_before();
+        __syncwarp();
+        if (lane == 0) ptx::mbar_arrive(o_ready);
     }
 }
 
-// ---- softmax warpgroup: all of Alg. 1 lines 4-9 and 12 for one 128-row tile ----------------------
-template <int EB, bool FOLD, int QKG>
-__device__ __forceinline__ void prefill_softmax(const FwdParams& p, int t, int wq, int lane, uint32_t tbase,
-                                                uint64_t* s_full, uint64_t* p_full, uint64_t* o_done, int n_t,
-                                                int row0, int bh, int kvh) {
+// ---- softmax warp (wq, half): Alg. 1 lines 4-9 and 12 for its rows of both tiles, its 64 key columns ----
+template <int EB, bool FOLD, bool AUX>
+__device__ __forceinline__ void prefill_softmax(const FwdParams& p, int wq, int half, int lane, uint32_t tbase,
+                                                 uint64_t* s_full, uint64_t* p_full, uint64_t* a_full, float* alpha_s,
+                                                 float* mx, uint64_t* o_done, const int* n_tile, int n_it, int pair,
+                                                 int bh, int kvh, const CUtensorMap* mapO, uint8_t* stage0,
+                                                 uint8_t* stage1) {
     using C = PrefillCfg<EB>;
+    using C4 = PrefillKCfg<EB>;
     const uint32_t tlane = tbase + (static_cast<uint32_t>(wq * 32) << 16);
-    const uint32_t tS = tlane + C::TM_S + t * 128, tO = tlane + C::TM_O + t * 128;
-    const int qrow = row0 + wq * 32 + lane;
+    const int rl = wq * 32 + lane;              // row within the tile = TMEM lane
     const int off = p.Lk - p.Lq;
-    long long jl = p.causal ? (long long)qrow + off : (long long)p.Lk - 1;
-    if (jl > p.Lk - 1) jl = p.Lk - 1;
-    const int jlim = (int)jl;
-    // first key index that some row of this warp cannot see (blocks reaching it need the masked path)
-    const int warp_first_row = row0 + wq * 32;
-    const long long warp_vis = p.causal ? (long long)warp_first_row + off : (long long)p.Lk - 1;
+    const int bar_id = 1 + wq;                  // named barrier of the two warps that share these rows
 
     float c_nat = p.sm_scale, vs = 1.0f;
     if constexpr (EB == 1) {
@@ -153,149 +99,177 @@ __device__ __forceinline__ void prefill_softmax(const FwdParams& p, int t, int w
     const float log2S = FOLD ? log2f(p.S) : 0.0f;   // exact for S = 2^k
     const uint64_t cl2_2 = ptx::pack2(cl2, cl2), s_2 = ptx::pack2(p.S, p.S);
 
-    float m_run = -INFINITY, l_run = 0.0f;   // l_run carries the factor S when FOLD
-    for (int c = 0; c < n_t; ++c) {
-        const int blk = (p.kv_order == 0) ? c : n_t - 1 - c;
-        const int j0 = blk * C::BN;
-        const bool mask = (j0 + C::BN - 1 > warp_vis) || (j0 + C::BN > p.Lk);
-        // ---- lines 4-5: block max, running max.  S arrives in four 32-column quarters ----
-        float mloc = -INFINITY;
-        {
-            uint32_t va[32], vb[32];
+    int jlim[2], first[2];
+    uint8_t* dump_row[2];     // AUX: this row of the P dump (fp8attn_stats.p_codes), else null
+    uint32_t uf_sink = 0, uf_other = 0;   // AUX: zero codes among visible non-sink keys (sink block / other blocks)
+    int mask_from[2];         // blocks whose first key index exceeds this need the mask for some row of the warp
+    float m_run[2] = {-INFINITY, -INFINITY}, l_run[2] = {0.0f, 0.0f};
 #pragma unroll
-            for (int h = 0; h < 2; ++h) {
-                if constexpr (QKG == 4) {
-                    ptx::mbar_wait(s_full + 2 * h, c & 1);
-                    ptx::tc_fence_after();
-                    ptx::tmem_ld_x32(tS + h * 64, va);
-                    ptx::mbar_wait(s_full + 2 * h + 1, c & 1);
-                    ptx::tc_fence_after();
-                } else {
-                    if (QKG == 2 || h == 0) {
-                        ptx::mbar_wait(s_full + (QKG == 2 ? h : 0), c & 1);
-                        ptx::tc_fence_after();
-                    }
-                    ptx::tmem_ld_x32(tS + h * 64, va);
-                }
-                ptx::tmem_ld_x32(tS + h * 64 + 32, vb);
-                ptx::tmem_wait_ld();
-                if (mask) {
-#pragma unroll
-                    for (int e = 0; e < 32; ++e) {
-                        if (j0 + h * 64 + e > jlim) va[e] = 0xFF800000u;
-                        if (j0 + h * 64 + 32 + e > jlim) vb[e] = 0xFF800000u;
-                    }
-                }
-                float m0 = mloc, m1 = -INFINITY;
-#pragma unroll
-                for (int e = 0; e < 32; e += 2) {
-                    m0 = fmaxf(fmaxf(m0, __uint_as_float(va[e])), __uint_as_float(va[e + 1]));
-                    m1 = fmaxf(fmaxf(m1, __uint_as_float(vb[e])), __uint_as_float(vb[e + 1]));
-                }
-                mloc = fmaxf(m0, m1);
-            }
-        }
-        const float m_new = fmaxf(m_run, mloc);
-        const float m_used = (m_new == -INFINITY) ? 0.0f : m_new;
-        const float alpha = ptx::ex2_approx((m_run - m_used) * cl2);   // line 6 (0 when m_run = -inf)
-        const float negm = fmaf(-m_used, cl2, log2S);
-        const uint64_t negm_2 = ptx::pack2(negm, negm);
+    for (int t = 0; t < 2; ++t) {
+        const int row0 = (pair * 2 + t) * BM;
+        long long jl = p.causal ? (long long)row0 + rl + off : (long long)p.Lk - 1;
+        if (jl > p.Lk - 1) jl = p.Lk - 1;
+        jlim[t] = (int)jl;
+        // a block j0 .. j0 + 127 is unmasked iff every row of the warp sees all of it and it lies inside Lk
+        const long long wvis = p.causal ? (long long)row0 + wq * 32 + off : (long long)p.Lk - 1;
+        long long thr = wvis - 127 < (long long)p.Lk - 128 ? wvis - 127 : (long long)p.Lk - 128;
+        if (thr < -(1ll << 30)) thr = -(1ll << 30);
+        mask_from[t] = (int)thr;
+        first[t] = (p.kv_order == 0) ? 0 : n_it - n_tile[t];
+        dump_row[t] = (AUX && p.p_codes != nullptr && bh == p.p_bh && row0 + rl < p.Lq)
+                          ? p.p_codes + (size_t)(row0 + rl) * p.Lk
+                          : nullptr;
+    }
 
-        // ---- line 10, first half: O <- alpha O.  S(c) complete implies PV(c-1) complete (in-order pipe) ----
-        if (c > 0 && __any_sync(0xFFFFFFFFu, alpha != 1.0f)) {
-            const uint64_t a2 = ptx::pack2(alpha, alpha);
+    // A successful mbarrier wait takes ~130 cycles to report.  When the next block belongs to the other tile its
+    // S has been ready for a while, so the barrier is probed before the second P quarter of the current block
+    // and the answer is read when the next block starts (probed_tile >= 0: a probe is pending).
+    FP8ATTN_DECL_PROBE_PRED();
+    int probed_tile = -1;
 #pragma unroll 1
-            for (int hb = 0; hb < 2; ++hb) {
-                uint32_t v[64];
-                ptx::tmem_ld_x32(tO + hb * 64, v);
-                ptx::tmem_ld_x32(tO + hb * 64 + 32, v + 32);
-                ptx::tmem_wait_ld();
+    for (int it = 0; it < n_it; ++it) {
 #pragma unroll
-                for (int e = 0; e < 64; e += 2) {
-                    float y0, y1;
-                    ptx::unpack2(ptx::mul2(ptx::pack2u(v[e], v[e + 1]), a2), y0, y1);
-                    v[e] = __float_as_uint(y0);
-                    v[e + 1] = __float_as_uint(y1);
-                }
-                ptx::tmem_st_x32(tO + hb * 64, v);
-                ptx::tmem_st_x32(tO + hb * 64 + 32, v + 32);
-            }
-        }
-
-        // ---- lines 7-9: P = exp(Z - m), l from the pre-cast P, cast, P -> TMEM over S ----
-        uint64_t sum_a = ptx::pack2(0.f, 0.f), sum_b = sum_a;
-        {
-            uint32_t va[32], vb[32], w[C::P_COLS / 4];
-            ptx::tmem_ld_x32(tS, va);
+        for (int tt = 0; tt < 2; ++tt) {
+            const int t = 1 - tt;               // tile 1 first: under a causal mask it has the extra block
+            const int c = it - first[t];
+            if (c < 0 || c >= n_tile[t]) continue;
+            // the block after this one, if it is a block of the other tile
+            const int it_o = it + tt;           // tile 1 -> (it, tile 0);  tile 0 -> (it + 1, tile 1)
+            const int c_o = it_o - first[t ^ 1];
+            const bool probe_next = c_o >= 0 && c_o < n_tile[t ^ 1];
+            const int blk = (p.kv_order == 0) ? c : n_tile[t] - 1 - c;
+            const int j0 = blk * 128;
+            const bool mask = j0 > mask_from[t];
+            const uint32_t tS = tlane + C::TM_S + t * 128;
+            // ---- this warp's 64 logits of the row, loaded once ----
+            uint32_t r[64];
+            if (probed_tile != t || !ptx::mbar_probe_result()) ptx::mbar_wait(s_full + t, c & 1);
+            probed_tile = -1;
+            ptx::tc_fence_after();
+            ptx::tmem_ld_x32(tS + half * 64, r);
+            ptx::tmem_ld_x32(tS + half * 64 + 32, r + 32);
             ptx::tmem_wait_ld();
-#pragma unroll
-            for (int cb = 0; cb < 4; ++cb) {
-                uint32_t* cur = (cb & 1) ? vb : va;
-                uint32_t* nxt = (cb & 1) ? va : vb;
-                if (cb < 3) ptx::tmem_ld_x32(tS + (cb + 1) * 32, nxt);
-                if (mask)
-                    exp_chunk<EB, FOLD, true>(cur, w, j0 + cb * 32, jlim, cl2_2, negm_2, s_2, sum_a, sum_b);
-                else
-                    exp_chunk<EB, FOLD, false>(cur, w, j0 + cb * 32, jlim, cl2_2, negm_2, s_2, sum_a, sum_b);
-                // P quarter over the head of its own S quarter; the P.V of this quarter can start at once
-                if constexpr (EB == 1) ptx::tmem_st_x8(tS + cb * 32, w);
-                else ptx::tmem_st_x16(tS + cb * 32, w);
-                ptx::tmem_wait_st();       // (also covers the O rescale stores before the first quarter)
-                ptx::tc_fence_before();
+            if (mask) {
+                mask32(r, j0 + half * 64, jlim[t]);
+                mask32(r + 32, j0 + half * 64 + 32, jlim[t]);
+            }
+            // ---- lines 4-6: block max (exchanged with the warp of the other column half), running max ----
+            float mloc = fmaxf(max32(r, -INFINITY), max32(r + 32, -INFINITY));
+            float* mxt = mx + (t * 2 + (c & 1)) * 256;
+            mxt[half * 128 + rl] = mloc;
+            ptx::named_bar_sync(bar_id, 64);
+            mloc = fmaxf(mloc, mxt[(half ^ 1) * 128 + rl]);
+            const float m_new = fmaxf(m_run[t], mloc);
+            const float m_used = (m_new == -INFINITY) ? 0.0f : m_new;
+            const float alpha = ptx::ex2_approx((m_run[t] - m_used) * cl2);   // 0 when m_run = -inf
+            const float negm = fmaf(-m_used, cl2, log2S);
+            const uint64_t negm_2 = ptx::pack2(negm, negm);
+            if (half == 0) {                    // alpha goes to the correction warp of these rows
+                alpha_s[t * 128 + rl] = alpha;
                 __syncwarp();
-                if (lane == 0) ptx::mbar_arrive(p_full + cb);
-                if (cb < 3) ptx::tmem_wait_ld();
+                if (lane == 0) ptx::mbar_arrive(a_full + 4 * t + wq);
             }
+            // ---- lines 7-9: two P quarters ----
+            uint64_t sum_a = ptx::pack2(0.f, 0.f), sum_b = sum_a;
+            // (a masked logit is -inf: exp2_poly2 turns it into 2^-125, which casts to the E4M3 code 0 and is
+            // far below one ulp of a row sum that holds a visible key; rows without any visible key are set to
+            // l = 0 in the epilogue)
+            // AUX: the counter this block adds to (blocks that hold a sink key / all others); rows >= Lq do not
+            // exist and are not counted
+            uint32_t* const uf = (AUX && p.underflow != nullptr && (pair * 2 + t) * BM + rl < p.Lq)
+                                     ? (j0 < p.n_sink ? &uf_sink : &uf_other)
+                                     : nullptr;
+            p_quarter<EB, FOLD, C4::NPOLY, AUX>(r, false, tS, 2 * half, j0, jlim[t], cl2_2, negm_2, s_2, sum_a, sum_b,
+                                                p_full + 2 * t + 0, lane, dump_row[t], uf, p.n_sink);
+            if (probe_next) {
+                ptx::mbar_probe(s_full + (t ^ 1), c_o & 1);
+                probed_tile = t ^ 1;
+            }
+            p_quarter<EB, FOLD, C4::NPOLY, AUX>(r + 32, false, tS, 2 * half + 1, j0, jlim[t], cl2_2, negm_2, s_2, sum_a,
+                                                sum_b, p_full + 2 * t + 1, lane, dump_row[t], uf, p.n_sink);
+            float sa, sb, sc, sd;
+            ptx::unpack2(sum_a, sa, sb);
+            ptx::unpack2(sum_b, sc, sd);
+            l_run[t] = alpha * l_run[t] + ((sa + sb) + (sc + sd));   // line 8 (this warp's columns)
+            m_run[t] = m_new;
         }
-        float sa, sb, sc, sd;
-        ptx::unpack2(sum_a, sa, sb);
-        ptx::unpack2(sum_b, sc, sd);
-        l_run = alpha * l_run + ((sa + sb) + (sc + sd));   // line 8
-        m_run = m_new;
     }
 
-    // ---- line 12: O / (S l), statistics ----
-    const long long grow = (long long)bh * p.Lq + qrow;
-    const float l_true = FOLD ? l_run / p.S : l_run;
-    if (qrow < p.Lq) {
-        if (p.row_max) p.row_max[grow] = (m_run == -INFINITY) ? -INFINITY : m_run * c_nat;
-        if (p.row_sum) p.row_sum[grow] = l_true;
-    }
-    const float inv = (l_run > 0.0f) ? (FOLD ? vs / l_run : vs / (p.S * l_run)) : 0.0f;
-    if (n_t > 0) {
-        ptx::mbar_wait(o_done, 0);
-        ptx::tc_fence_after();
-    }
-    float* dst = p.o + grow * C::D;
-#pragma unroll 1
-    for (int cb = 0; cb < 4; ++cb) {
-        uint32_t v[32];
-        if (n_t > 0) {
-            ptx::tmem_ld_x32(tO + cb * 32, v);
-            ptx::tmem_wait_ld();
-        } else {
-#pragma unroll
-            for (int e = 0; e < 32; ++e) v[e] = 0u;
-        }
-        if (qrow < p.Lq) {
-#pragma unroll
-            for (int e = 0; e < 32; e += 4) {
-                float4 o4 = make_float4(__uint_as_float(v[e]) * inv, __uint_as_float(v[e + 1]) * inv,
-                                        __uint_as_float(v[e + 2]) * inv, __uint_as_float(v[e + 3]) * inv);
-                if (l_run <= 0.0f) o4 = make_float4(0.f, 0.f, 0.f, 0.f);
-                *reinterpret_cast<float4*>(dst + cb * 32 + e) = o4;
+    if constexpr (AUX) {
+        if (p.underflow != nullptr) {       // one atomic per warp and counter (ballot / popc style reduction)
+            const uint32_t a = __reduce_add_sync(0xFFFFFFFFu, uf_sink), b2 = __reduce_add_sync(0xFFFFFFFFu, uf_other);
+            if (lane == 0) {
+                if (a) atomicAdd(p.underflow + 0, (unsigned long long)a);
+                if (b2) atomicAdd(p.underflow + 1, (unsigned long long)b2);
             }
         }
+    }
+    // ---- line 12: O / (S l), statistics.  Each warp owns 32 rows x 64 output columns of each tile: it scales
+    // them, writes them as two 32-row x 128-byte boxes (128-byte swizzle) into the K / V ring, which no MMA reads
+    // any more once both tiles are done, and stores the boxes with TMA (rows >= Lq are clipped by the map) ----
+#pragma unroll
+    for (int t = 0; t < 2; ++t) {
+        if (n_tile[t] > 0) ptx::mbar_wait(o_done + t, 0);
+    }
+    ptx::tc_fence_after();
+#pragma unroll
+    for (int t = 0; t < 2; ++t) {
+        const int row0 = (pair * 2 + t) * BM;
+        const int qrow = row0 + rl;
+        const long long grow = (long long)bh * p.Lq + qrow;
+        float* mxt = mx + t * 512;
+        ptx::named_bar_sync(bar_id, 64);        // the partner has read the last block maximum
+        const float l_mine = (m_run[t] == -INFINITY) ? 0.0f : l_run[t];   // no visible key: l = 0 exactly
+        mxt[half * 128 + rl] = l_mine;
+        ptx::named_bar_sync(bar_id, 64);
+        const float l_all = l_mine + mxt[(half ^ 1) * 128 + rl];
+        const float l_true = FOLD ? l_all / p.S : l_all;
+        if (qrow < p.Lq && half == 0) {
+            if (p.row_max) p.row_max[grow] = (m_run[t] == -INFINITY) ? -INFINITY : m_run[t] * c_nat;
+            if (p.row_sum) p.row_sum[grow] = l_true;
+        }
+        const float inv = (l_all > 0.0f) ? (FOLD ? vs / l_all : vs / (p.S * l_all)) : 0.0f;
+        if (row0 >= p.Lq) continue;             // no row of this tile exists (warp-uniform)
+        const uint32_t tO = tlane + C::TM_O + t * 128 + half * 64;
+        uint8_t* stage = t ? stage1 : stage0;
+#pragma unroll 1
+        for (int cb = 0; cb < 2; ++cb) {
+            const int ch = half * 2 + cb;       // 32-column chunk of the output row
+            uint32_t v[32];
+            if (n_tile[t] > 0) {
+                ptx::tmem_ld_x32(tO + cb * 32, v);
+                ptx::tmem_wait_ld();
+            } else {
+#pragma unroll
+                for (int e = 0; e < 32; ++e) v[e] = 0u;
+            }
+            uint8_t* box = stage + (ch * 4 + wq) * 4096;
+#pragma unroll
+            for (int j = 0; j < 8; ++j) {
+                const float4 o4 = make_float4(__uint_as_float(v[4 * j]) * inv, __uint_as_float(v[4 * j + 1]) * inv,
+                                              __uint_as_float(v[4 * j + 2]) * inv, __uint_as_float(v[4 * j + 3]) * inv);
+                *reinterpret_cast<float4*>(box + lane * 128 + ((j ^ (lane & 7)) << 4)) = o4;
+            }
+            ptx::fence_proxy_async_smem();
+            __syncwarp();
+            if (lane == 0) ptx::tma_store_3d(mapO, box, ch * 32, row0 + wq * 32, bh);
+        }
+    }
+    if (lane == 0) {
+        ptx::bulk_commit_group();
+        ptx::bulk_wait_group_read0();
     }
 }
 
 // ---- the kernel ---------------------------------------------------------------------------------
-// grid = (ceil(Lq / 256), B*Hq).  Causal launches the heaviest tile pairs first.
-template <int EB, bool FOLD, int QKG>
-__global__ void __launch_bounds__(352, 1)
+// grid = ceil(Lq / 256) * B*Hq CTAs in one dimension (order: see below).
+template <int EB, bool FOLD, bool AUX = false>
+__global__ void __launch_bounds__(640, 1)
 attn_prefill_kernel(const __grid_constant__ CUtensorMap mapQ, const __grid_constant__ CUtensorMap mapK,
-                    const __grid_constant__ CUtensorMap mapV, const FwdParams p) {
+                     const __grid_constant__ CUtensorMap mapV, const __grid_constant__ CUtensorMap mapO,
+                     const FwdParams p) {
     using C = PrefillCfg<EB>;
+    using C4 = PrefillKCfg<EB>;
     extern __shared__ uint8_t smem_raw[];
     uint8_t* smem = reinterpret_cast<uint8_t*>((reinterpret_cast<uintptr_t>(smem_raw) + 1023) & ~uintptr_t(1023));
     uint8_t* sQ = smem;                           // 2 tiles
@@ -307,15 +281,27 @@ attn_prefill_kernel(const __grid_constant__ CUtensorMap mapQ, const __grid_const
     uint64_t* k_empty = k_full + C::NS;
     uint64_t* v_full = k_empty + C::NS;
     uint64_t* v_empty = v_full + C::NS;
-    uint64_t* s_full = v_empty + C::NS;           // [2 tiles][4 quarters]  MMA -> softmax
-    uint64_t* p_full = s_full + 8;                // [2 tiles][4 quarters]  softmax (4 warps) -> MMA
-    uint64_t* o_done = p_full + 8;                // [2]
+    uint64_t* s_full = v_empty + C::NS;           // [2 tiles]                   MMA -> softmax
+    uint64_t* p_full = s_full + 2;                // [2 tiles][2 steps]          softmax (8 warps) -> MMA
+    uint64_t* a_full = p_full + 4;                // [2 tiles][4 warps]          softmax warp -> correction warp
+    uint64_t* o_ready = a_full + 8;               // [2]                         correction (4 warps) -> MMA
+    uint64_t* o_done = o_ready + 2;               // [2]
     uint32_t* tmem_slot = reinterpret_cast<uint32_t*>(o_done + 2);
+    float* alpha_s = reinterpret_cast<float*>(tmem_slot + 4);   // [2 tiles][128 rows]
+    float* mx = alpha_s + 256;                                  // [2 tiles][2 parities][2 halves][128 rows]
 
     const int tid = threadIdx.x, lane = tid & 31;
     const int warp = __shfl_sync(0xFFFFFFFFu, tid >> 5, 0);   // provably warp-uniform
-    const int pair = p.causal ? (int)(gridDim.x - 1 - blockIdx.x) : (int)blockIdx.x;
-    const int bh = blockIdx.y;
+    // 1-D grid, launch order = longest work first within groups of HEAD_GROUP (batch, q head) slabs: a group's
+    // K and V (2 x Lk x 128 B per kv head) stay in L2 while its CTAs run, and only the last group's lightest CTAs
+    // are left for the tail of the kernel.
+    const int n_pairs = (p.Lq + 2 * BM - 1) / (2 * BM), n_heads = p.B * p.Hq;
+    const int grp = (int)blockIdx.x / (C4::HEAD_GROUP * n_pairs);
+    const int rem = (int)blockIdx.x - grp * C4::HEAD_GROUP * n_pairs;
+    const int grp_size = min(C4::HEAD_GROUP, n_heads - grp * C4::HEAD_GROUP);
+    const int pair_idx = rem / grp_size;
+    const int pair = p.causal ? n_pairs - 1 - pair_idx : pair_idx;
+    const int bh = grp * C4::HEAD_GROUP + rem % grp_size;
     const int b = bh / p.Hq, h = bh % p.Hq;
     const int kvh = b * p.Hkv + h / (p.Hq / p.Hkv);
 
@@ -341,6 +327,7 @@ attn_prefill_kernel(const __grid_constant__ CUtensorMap mapQ, const __grid_const
         ptx::prefetch_tmap(&mapQ);
         ptx::prefetch_tmap(&mapK);
         ptx::prefetch_tmap(&mapV);
+        ptx::prefetch_tmap(&mapO);
         for (int i = 0; i < 2; ++i) ptx::mbar_init(q_full + i, 1);
         for (int i = 0; i < C::NS; ++i) {
             ptx::mbar_init(k_full + i, 1);
@@ -348,15 +335,16 @@ attn_prefill_kernel(const __grid_constant__ CUtensorMap mapQ, const __grid_const
             ptx::mbar_init(k_empty + i, 2);   // one arrival per tile
             ptx::mbar_init(v_empty + i, 2);
         }
-        for (int i = 0; i < 8; ++i) {
+        for (int i = 0; i < 2; ++i) {
             ptx::mbar_init(s_full + i, 1);
-            ptx::mbar_init(p_full + i, 4);
+            ptx::mbar_init(o_ready + i, 4);
+            ptx::mbar_init(o_done + i, 1);
         }
-        ptx::mbar_init(o_done + 0, 1);
-        ptx::mbar_init(o_done + 1, 1);
+        for (int i = 0; i < 4; ++i) ptx::mbar_init(p_full + i, 8);
+        for (int i = 0; i < 8; ++i) ptx::mbar_init(a_full + i, 1);
         ptx::fence_mbar_init();
     }
-    if (warp == 8) {
+    if (warp == 16) {
         __syncwarp();
         ptx::tmem_alloc(tmem_slot, 512);
     }
@@ -366,127 +354,125 @@ attn_prefill_kernel(const __grid_constant__ CUtensorMap mapQ, const __grid_const
     const uint32_t tbase = *tmem_slot;
 
     if (warp < 8) {
-        const int t = warp >> 2;
-        prefill_softmax<EB, FOLD, QKG>(p, t, warp & 3, lane, tbase, s_full + 4 * t, p_full + 4 * t, o_done + t,
-                                  n_tile[t], (pair * 2 + t) * BM, bh, kvh);
-    } else if (warp == 10) {
-        // ================= TMA producer =================
-        if (lane == 0 && n_it > 0) {
-            for (int t = 0; t < 2; ++t) {
-                if (n_tile[t] == 0) continue;
-                ptx::mbar_arrive_expect_tx(q_full + t, C::TILE);
-                for (int c = 0; c < C::NCH; ++c)
-                    ptx::tma_load_3d(sQ + t * C::TILE + c * (128 * 128), &mapQ, q_full + t, c * C::CH,
-                                     (pair * 2 + t) * BM, bh);
+        ptx::setmaxnreg_inc<C4::REG_SOFTMAX>();
+        prefill_softmax<EB, FOLD, AUX>(p, warp & 3, warp >> 2, lane, tbase, s_full, p_full, a_full, alpha_s, mx, o_done,
+                                   n_tile, n_it, pair, bh, kvh, &mapO, sK, sV);
+    } else if (warp < 16) {
+        ptx::setmaxnreg_dec<C4::REG_CORR>();
+        const int t = (warp - 8) >> 2, wq = warp & 3;
+        prefill_correction(t, wq, lane, tbase, a_full + 4 * t + wq, alpha_s + t * 128 + wq * 32 + lane, o_ready + t,
+                            n_tile[t]);
+    } else {
+        ptx::setmaxnreg_dec<C4::REG_MISC>();
+        if (warp == 18) {
+            // ================= TMA producer =================
+            if (lane == 0 && n_it > 0) {
+                for (int t = 0; t < 2; ++t) {
+                    if (n_tile[t] == 0) continue;
+                    ptx::mbar_arrive_expect_tx(q_full + t, C::TILE);
+                    for (int c = 0; c < C::NCH; ++c)
+                        ptx::tma_load_3d(sQ + t * C::TILE + c * (128 * 128), &mapQ, q_full + t, c * C::CH,
+                                         (pair * 2 + t) * BM, bh);
+                }
+                for (int it = 0; it < n_it; ++it) {
+                    const int blk = (p.kv_order == 0) ? it : n_it - 1 - it;
+                    const int st = it % C::NS;
+                    const uint32_t ph = (it / C::NS) & 1;
+                    ptx::mbar_wait(k_empty + st, ph ^ 1);
+                    ptx::mbar_arrive_expect_tx(k_full + st, C::TILE);
+                    for (int c = 0; c < C::NCH; ++c)
+                        ptx::tma_load_3d(sK + st * C::TILE + c * (128 * 128), &mapK, k_full + st, c * C::CH,
+                                         blk * C::BN, kvh);
+                    ptx::mbar_wait(v_empty + st, ph ^ 1);
+                    ptx::mbar_arrive_expect_tx(v_full + st, C::TILE);
+                    for (int c = 0; c < C::NCH; ++c)
+                        ptx::tma_load_3d(sV + st * C::TILE + c * (128 * 128), &mapV, v_full + st, c * C::CH,
+                                         blk * C::BN, kvh);
+                }
             }
-            for (int it = 0; it < n_it; ++it) {
-                const int blk = (p.kv_order == 0) ? it : n_it - 1 - it;
-                const int st = it % C::NS;
-                const uint32_t ph = (it / C::NS) & 1;
-                ptx::mbar_wait(k_empty + st, ph ^ 1);
-                ptx::mbar_arrive_expect_tx(k_full + st, C::TILE);
-                for (int c = 0; c < C::NCH; ++c)
-                    ptx::tma_load_3d(sK + st * C::TILE + c * (128 * 128), &mapK, k_full + st, c * C::CH,
-                                     blk * C::BN, kvh);
-                ptx::mbar_wait(v_empty + st, ph ^ 1);
-                ptx::mbar_arrive_expect_tx(v_full + st, C::TILE);
-                for (int c = 0; c < C::NCH; ++c)
-                    ptx::tma_load_3d(sV + st * C::TILE + c * (128 * 128), &mapV, v_full + st, c * C::CH,
-                                     blk * C::BN, kvh);
-            }
-        }
-    } else if (n_tile[warp - 8] > 0) {
-        // ================= MMA issuer of tile t = warp - 8 =================
-        // One issuer warp per tile, each blocking only on its own tile's barriers and on the K/V ring, so
-        // neither tile can hold up the other.  The whole warp runs the loop (warp-uniform control flow keeps
-        // descriptors and counters in uniform registers); one elected lane issues the MMAs and commits.
-        // Block c of tile t uses K/V ring iteration it = c + first (in reverse order the tile with fewer
-        // visible blocks joins later).  A ring slot is released by two arrivals, one per tile; on iterations
-        // that only one tile uses, that tile arrives twice.
-        const int t = warp - 8;
-        const int n_t = n_tile[t];
-        const bool leader = ptx::elect_one();
-        constexpr int NG = 128 / QKG;          // keys per QK^T group
-        constexpr int QPG = 4 / QKG;           // P quarters per QK^T group
-        constexpr uint32_t idesc_qk = ptx::make_idesc(C::FMT, C::FMT, ptx::MAJOR_K, ptx::MAJOR_K, BM, NG);
-        constexpr uint32_t idesc_pv = ptx::make_idesc(C::FMT, C::FMT, ptx::MAJOR_K, ptx::MAJOR_MN, BM, C::D);
-        constexpr uint32_t desc_hi = ptx::smem_desc_hi(1024);
-        const uint32_t q_lo = ptx::smem_desc_lo(ptx::smem_u32(sQ + t * C::TILE), 16);
-        const uint32_t k_lo = ptx::smem_desc_lo(ptx::smem_u32(sK), 16);
-        const uint32_t v_lo = ptx::smem_desc_lo(ptx::smem_u32(sV), C::BN * 128);
-        const uint32_t tS = tbase + C::TM_S + t * 128, tO = tbase + C::TM_O + t * 128;
-        const int first = (p.kv_order == 0) ? 0 : n_it - n_t;
-        const int n_other = n_tile[t ^ 1];
-        const int first_other = (p.kv_order == 0) ? 0 : n_it - n_other;
-        uint64_t* const sf = s_full + 4 * t;
-        uint64_t* const pf = p_full + 4 * t;
+        } else if (warp < 18 && n_tile[warp - 16] > 0) {
+            // ================= MMA issuer of tile t = warp - 16 =================
+            // Block c of tile t uses K/V ring iteration it = c + first.  A ring slot is released by two
+            // arrivals, one per tile; on iterations that only one tile uses, that tile arrives twice.
+            const int t = warp - 16;
+            const int n_t = n_tile[t];
+            const bool leader = ptx::elect_one();
+            constexpr uint32_t idesc_qk = ptx::make_idesc(C::FMT, C::FMT, ptx::MAJOR_K, ptx::MAJOR_K, BM, C::BN);
+            constexpr uint32_t idesc_pv = ptx::make_idesc(C::FMT, C::FMT, ptx::MAJOR_K, ptx::MAJOR_MN, BM, C::D);
+            constexpr uint32_t desc_hi = ptx::smem_desc_hi(1024);
+            const uint32_t q_lo = ptx::smem_desc_lo(ptx::smem_u32(sQ + t * C::TILE), 16);
+            const uint32_t k_lo = ptx::smem_desc_lo(ptx::smem_u32(sK), 16);
+            const uint32_t v_lo = ptx::smem_desc_lo(ptx::smem_u32(sV), C::BN * 128);
+            const uint32_t tS = tbase + C::TM_S + t * 128, tO = tbase + C::TM_O + t * 128;
+            const int first = (p.kv_order == 0) ? 0 : n_it - n_t;
+            const int n_other = n_tile[t ^ 1];
+            const int first_other = (p.kv_order == 0) ? 0 : n_it - n_other;
+            uint64_t* const pf = p_full + 2 * t;
 
-        // S_t[:, NG g .. NG (g+1)) = Q_t K[NG g .. NG (g+1), :]^T on ring iteration it
-        auto qk_group = [&](const int g, const int it) {
-            const int st = it % C::NS;
-            if (g == 0) {
+            // S_t = Q_t K^T on ring iteration it
+            auto qk_block = [&](const int it) {
+                const int st = it % C::NS;
                 ptx::mbar_wait(k_full + st, (it / C::NS) & 1);
                 ptx::tc_fence_after();
-            }
-            if (leader) {
-                const uint32_t b0 = k_lo + st * (C::TILE >> 4) + g * ((NG * 128) >> 4);
+                if (leader) {
+                    const uint32_t b0 = k_lo + st * (C::TILE >> 4);
 #pragma unroll
-                for (int ks = 0; ks < C::D / C::KSTEP; ++ks) {
-                    const uint32_t o = (((ks * 32) / 128) * (128 * 128) + (ks * 32) % 128) >> 4;
-                    ptx::mma_ss<C::KIND>(tS + g * NG, ptx::pack2u(q_lo + o, desc_hi), ptx::pack2u(b0 + o, desc_hi),
-                                         idesc_qk, ks > 0 ? 1u : 0u);
-                }
-                ptx::tc_commit(sf + g);
-                if (g == QKG - 1) {
+                    for (int ks = 0; ks < C::D / C::KSTEP; ++ks) {
+                        const uint32_t o = (((ks * 32) / 128) * (128 * 128) + (ks * 32) % 128) >> 4;
+                        ptx::mma_ss<C::KIND>(tS, ptx::pack2u(q_lo + o, desc_hi), ptx::pack2u(b0 + o, desc_hi), idesc_qk,
+                                             ks > 0 ? 1u : 0u);
+                    }
+                    ptx::tc_commit(s_full + t);
                     ptx::tc_commit(k_empty + st);
                     if (it < first_other || it >= first_other + n_other) ptx::tc_commit(k_empty + st);
                 }
-            }
-        };
-        // O_t += P_t[:, 32q .. 32q+32) V[32q .. 32q+32, :]
-        auto pv_group = [&](const int q, const int it, const uint32_t acc0, const bool last_of_tile) {
-            const int st = it % C::NS;
-            if (q == 0) {
-                ptx::mbar_wait(v_full + st, (it / C::NS) & 1);
-                ptx::tc_fence_after();
-            }
-            if (leader) {
-                const uint32_t b0 = v_lo + st * (C::TILE >> 4) + q * ((32 * 128) >> 4);
-                uint32_t acc = acc0;
+            };
+            // O_t += P_t[:, 32q .. 32q+32) V[32q .. 32q+32, :]
+            auto pv_quarter = [&](const int q, const int it, const uint32_t acc0) {
+                const int st = it % C::NS;
+                if (leader) {
+                    const uint32_t b0 = v_lo + st * (C::TILE >> 4) + q * ((32 * 128) >> 4);
+                    uint32_t acc = acc0;
 #pragma unroll
-                for (int ks = 0; ks < 32 / C::KSTEP; ++ks) {
-                    ptx::mma_ts<C::KIND>(tO, tS + q * 32 + ks * 8, ptx::pack2u(b0 + ks * ((C::KSTEP * 128) >> 4), desc_hi),
-                                         idesc_pv, acc);
-                    acc = 1;
+                    for (int ks = 0; ks < 32 / C::KSTEP; ++ks) {
+                        ptx::mma_ts<C::KIND>(tO, tS + q * 32 + ks * 8,
+                                             ptx::pack2u(b0 + ks * ((C::KSTEP * 128) >> 4), desc_hi), idesc_pv, acc);
+                        acc = 1;
+                    }
                 }
-                if (last_of_tile) ptx::tc_commit(o_done + t);
-                if (q == 3) {
+            };
+
+            ptx::mbar_wait(q_full + t, 0);
+            ptx::tc_fence_after();
+            qk_block(first);
+            for (int c = 0; c < n_t; ++c) {
+                const int it = c + first;
+                const int st = it % C::NS;
+                const bool has_next = c + 1 < n_t;
+                ptx::mbar_wait(v_full + st, (it / C::NS) & 1);
+                ptx::mbar_wait(o_ready + t, c & 1);
+                // first quarter of each column half, then the second one (the order the softmax warps write them)
+                ptx::mbar_wait(pf + 0, c & 1);
+                ptx::tc_fence_after();
+                pv_quarter(0, it, c > 0 ? 1u : 0u);
+                pv_quarter(2, it, 1u);
+                ptx::mbar_wait(pf + 1, c & 1);
+                ptx::tc_fence_after();
+                pv_quarter(1, it, 1u);
+                pv_quarter(3, it, 1u);
+                if (leader) {
+                    if (!has_next) ptx::tc_commit(o_done + t);
                     ptx::tc_commit(v_empty + st);
                     if (it < first_other || it >= first_other + n_other) ptx::tc_commit(v_empty + st);
                 }
-            }
-        };
-
-        ptx::mbar_wait(q_full + t, 0);
-        ptx::tc_fence_after();
-#pragma unroll
-        for (int g = 0; g < QKG; ++g) qk_group(g, first);
-        for (int c = 0; c < n_t; ++c) {
-            const int it = c + first;
-            const bool has_next = c + 1 < n_t;
-#pragma unroll
-            for (int q = 0; q < 4; ++q) {
-                ptx::mbar_wait(pf + q, c & 1);
-                ptx::tc_fence_after();
-                pv_group(q, it, (c > 0 || q > 0) ? 1u : 0u, !has_next && q == 3);
-                if (has_next && (q + 1) % QPG == 0) qk_group(q / QPG, it + 1);
+                if (has_next) qk_block(it + 1);
             }
         }
     }
 
     ptx::tc_fence_before();
     __syncthreads();
-    if (warp == 8) ptx::tmem_dealloc(tbase, 512);
+    if (warp == 16) ptx::tmem_dealloc(tbase, 512);
 }
 
 }  // namespace fp8attn

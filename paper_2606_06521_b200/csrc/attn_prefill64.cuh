@@ -15,7 +15,7 @@
 // Semantics as everywhere: exact running max after every block, l from the FP32 pre-cast P (line 8), P*S
 // cast with cvt.rn.satfinite.e4m3x2.f32 (line 9), O / (S l) at the end (line 12).
 #pragma once
-#include "attn_prefill.cuh"
+#include "prefill_common.cuh"
 
 namespace fp8attn {
 
@@ -51,7 +51,7 @@ struct Softmax64Shared {
 };
 static_assert(sizeof(Softmax64Shared) == 6144, "SMEM_BYTES accounts for 6144 bytes");
 
-template <int EB, bool FOLD>
+template <int EB, bool FOLD, bool AUX>
 __device__ __forceinline__ void prefill64_softmax(const FwdParams& p, int t, int par, int wq, int lane, uint32_t tbase,
                                                   uint64_t* s_full, uint64_t* p_full, uint64_t* pv_done,
                                                   uint64_t* o_done, uint64_t* m_full, int n_t, int row0, int bh,
@@ -79,6 +79,11 @@ __device__ __forceinline__ void prefill64_softmax(const FwdParams& p, int t, int
     const uint64_t cl2_2 = ptx::pack2(cl2, cl2), s_2 = ptx::pack2(p.S, p.S);
 
     float m_own = -INFINITY, l_own = 0.0f;   // partial sum of this warp's blocks, relative to m_own; carries S when FOLD
+    // statistics instance: this row of the P dump, and the zero codes among visible non-sink keys
+    uint8_t* const dump_row = (AUX && p.p_codes != nullptr && bh == p.p_bh && qrow < p.Lq)
+                                  ? p.p_codes + (size_t)qrow * p.Lk : nullptr;
+    const bool count = AUX && p.underflow != nullptr && qrow < p.Lq;
+    uint32_t uf_sink = 0, uf_other = 0;
     for (int c = par; c < n_t; c += 2) {
         const int blk = (p.kv_order == 0) ? c : n_t - 1 - c;
         const int j0 = blk * C::BN;
@@ -133,6 +138,9 @@ __device__ __forceinline__ void prefill64_softmax(const FwdParams& p, int t, int
             ptx::tmem_wait_ld();
             if (mask) exp_chunk<EB, FOLD, true>(v, w, j0 + cb * 32, jlim, cl2_2, negm_2, s_2, sum_a, sum_b);
             else exp_chunk<EB, FOLD, false>(v, w, j0 + cb * 32, jlim, cl2_2, negm_2, s_2, sum_a, sum_b);
+            if constexpr (AUX)
+                chunk_statistics<EB>(w, j0 + cb * 32, jlim, dump_row,
+                                     count ? (j0 < p.n_sink ? &uf_sink : &uf_other) : nullptr, p.n_sink);
             // (P of chunk cb lands on columns of chunk 0, whose logits are already in registers)
             if constexpr (EB == 1) ptx::tmem_st_x8(tS + cb * 8, w);
             else ptx::tmem_st_x16(tS + cb * 16, w);
@@ -169,6 +177,15 @@ __device__ __forceinline__ void prefill64_softmax(const FwdParams& p, int t, int
         if (lane == 0) ptx::mbar_arrive(p_full + par);
     }
 
+    if constexpr (AUX) {
+        if (p.underflow != nullptr) {       // one atomic per warp and counter
+            const uint32_t a = __reduce_add_sync(0xFFFFFFFFu, uf_sink), b2 = __reduce_add_sync(0xFFFFFFFFu, uf_other);
+            if (lane == 0) {
+                if (a) atomicAdd(p.underflow + 0, (unsigned long long)a);
+                if (b2) atomicAdd(p.underflow + 1, (unsigned long long)b2);
+            }
+        }
+    }
     // ---- merge the two partial row sums; line 12: O / (S l), statistics ----
     sh->l[t][par][r] = l_own;
     sh->mlast[t][par][r] = m_own;
@@ -211,8 +228,9 @@ __device__ __forceinline__ void prefill64_softmax(const FwdParams& p, int t, int
 }
 
 // ---- the kernel ---------------------------------------------------------------------------------
-// grid = (ceil(Lq / 256), B*Hq).  Causal launches the heaviest tile pairs first.
-template <int EB, bool FOLD>
+// grid = ceil(Lq / 256) * B*Hq CTAs in one dimension, tile pair fastest.  Causal launches the heaviest tile pairs
+// first.  AUX: the statistics instance (P dump, underflow counters), same schedule.
+template <int EB, bool FOLD, bool AUX = false>
 __global__ void __launch_bounds__(608, 1)
 attn_prefill64_kernel(const __grid_constant__ CUtensorMap mapQ, const __grid_constant__ CUtensorMap mapK,
                       const __grid_constant__ CUtensorMap mapV, const FwdParams p) {
@@ -238,8 +256,10 @@ attn_prefill64_kernel(const __grid_constant__ CUtensorMap mapQ, const __grid_con
 
     const int tid = threadIdx.x, lane = tid & 31;
     const int warp = __shfl_sync(0xFFFFFFFFu, tid >> 5, 0);   // provably warp-uniform
-    const int pair = p.causal ? (int)(gridDim.x - 1 - blockIdx.x) : (int)blockIdx.x;
-    const int bh = blockIdx.y;
+    const int n_pairs = (p.Lq + 2 * BM - 1) / (2 * BM);
+    const int pair_idx = (int)(blockIdx.x % n_pairs);
+    const int pair = p.causal ? n_pairs - 1 - pair_idx : pair_idx;
+    const int bh = (int)(blockIdx.x / n_pairs);
     const int b = bh / p.Hq, h = bh % p.Hq;
     const int kvh = b * p.Hkv + h / (p.Hq / p.Hkv);
 
@@ -294,7 +314,7 @@ attn_prefill64_kernel(const __grid_constant__ CUtensorMap mapQ, const __grid_con
 
     if (warp < 16) {
         const int t = warp >> 3, wq = warp & 3;
-        prefill64_softmax<EB, FOLD>(p, t, (warp >> 2) & 1, wq, lane, tbase, s_full + 2 * t, p_full + 2 * t, pv_done + t,
+        prefill64_softmax<EB, FOLD, AUX>(p, t, (warp >> 2) & 1, wq, lane, tbase, s_full + 2 * t, p_full + 2 * t, pv_done + t,
                                     o_done + t, m_full + (t * 4 + wq) * 2, n_tile[t], (pair * 2 + t) * BM, bh, kvh, sh);
     } else if (warp == 18) {
         // ================= TMA producer =================

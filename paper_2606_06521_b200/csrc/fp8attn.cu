@@ -9,11 +9,11 @@
 #include <mutex>
 
 #include "../../include/fp8attn.h"
+#include <atomic>
+
 #include "attn_general.cuh"
 #include "attn_prefill.cuh"
 #include "attn_prefill64.cuh"
-#include "attn_prefill3.cuh"
-#include "attn_prefill4.cuh"
 #include "attn_decode.cuh"
 #include "debug_gemm.cuh"
 #include "prep.cuh"
@@ -104,33 +104,85 @@ int make_map(CUtensorMap* m, const void* base, int eb, long long slabs, long lon
     return FP8ATTN_OK;
 }
 
-// ---------------------------------------------------------------------------- scratch memory
-// One growing stream-ordered buffer per purpose.  Freed and reallocated on the caller's stream,
-// so no host synchronisation is needed; kernels already enqueued keep their memory until they ran.
-struct Scratch {
+// ---------------------------------------------------------------------------- per-device state, scratch memory
+// Scratch (split-KV partials, BF16 planes of FP32 inputs, the quantised q of a decode call, the staging of
+// fp8attn_fwd_host) is allocated PER CALL from a library-owned stream-ordered memory pool of the current device,
+// on the caller's stream, and freed on that stream once the call's kernels are enqueued.  Two calls therefore
+// never share scratch, whatever streams or devices they run on, and nothing is freed while a kernel that uses it
+// is pending.  The pool keeps freed memory (release threshold = max), so steady-state calls do not reach the OS.
+constexpr int MAX_DEVICES = 64;
+struct DeviceState {
+    std::mutex mu;           // guards `pool`
+    cudaMemPool_t pool = nullptr;
+    // fp8attn_fwd_host: two copy streams and the events that chain the pieces; host calls on one device take
+    // turns (host_mu), each synchronises its stream before it returns anyway
+    std::mutex host_mu;
+    cudaStream_t s_in = nullptr, s_out = nullptr;
+    cudaEvent_t ev_start = nullptr, ev_in[8] = {}, ev_done[8] = {};
+};
+DeviceState g_dev[MAX_DEVICES];
+
+int current_device(int* dev) {
+    if (cudaGetDevice(dev) != cudaSuccess || *dev < 0 || *dev >= MAX_DEVICES) {
+        cudaGetLastError();
+        set_err("no usable CUDA device");
+        return FP8ATTN_E_DEVICE;
+    }
+    return FP8ATTN_OK;
+}
+
+int device_pool(cudaMemPool_t* out) {
+    int dev = 0;
+    if (int rc = current_device(&dev)) return rc;
+    DeviceState& d = g_dev[dev];
+    std::lock_guard<std::mutex> lock(d.mu);
+    if (!d.pool) {
+        cudaMemPoolProps props;
+        memset(&props, 0, sizeof props);
+        props.allocType = cudaMemAllocationTypePinned;
+        props.handleTypes = cudaMemHandleTypeNone;
+        props.location.type = cudaMemLocationTypeDevice;
+        props.location.id = dev;
+        CU_TRY(cudaMemPoolCreate(&d.pool, &props));
+        unsigned long long keep = ~0ull;
+        CU_TRY(cudaMemPoolSetAttribute(d.pool, cudaMemPoolAttrReleaseThreshold, &keep));
+    }
+    *out = d.pool;
+    return FP8ATTN_OK;
+}
+
+// One allocation, returned to the pool on `st` when the lease goes out of scope.
+struct Lease {
     void* ptr = nullptr;
-    size_t bytes = 0;
-    int dev = -1;
-    int get(void** out, size_t need, cudaStream_t st) {
-        int dev_now = 0;
-        cudaGetDevice(&dev_now);
-        if (ptr && (dev_now != dev || need > bytes)) {
-            cudaFreeAsync(ptr, st);
-            ptr = nullptr;
-            bytes = 0;
-        }
-        if (!ptr) {
-            size_t sz = need < 256 ? 256 : need;
-            CU_TRY(cudaMallocAsync(&ptr, sz, st));
-            bytes = sz;
-            dev = dev_now;
-        }
-        *out = ptr;
+    cudaStream_t st = nullptr;
+    Lease() = default;
+    Lease(const Lease&) = delete;
+    Lease& operator=(const Lease&) = delete;
+    ~Lease() {
+        if (ptr) cudaFreeAsync(ptr, st);
+    }
+    int get(size_t bytes, cudaStream_t stream) {
+        cudaMemPool_t pool;
+        if (int rc = device_pool(&pool)) return rc;
+        st = stream;
+        CU_TRY(cudaMallocFromPoolAsync(&ptr, bytes < 256 ? 256 : bytes, pool, stream));
         return FP8ATTN_OK;
     }
 };
-std::mutex g_mu;                      // serialises calls that use the scratch buffers
-Scratch g_planes, g_partial, g_qquant, g_amax;
+
+// Opt a kernel in to more than 48 KB of dynamic shared memory: the attribute is per device, `done` holds one
+// bit per device (one static mask per kernel instance).
+template <typename K>
+int ensure_smem(K kern, int bytes, std::atomic<unsigned long long>& done) {
+    int dev = 0;
+    if (int rc = current_device(&dev)) return rc;
+    const unsigned long long bit = 1ull << dev;
+    if (!(done.load(std::memory_order_acquire) & bit)) {
+        CU_TRY(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes));
+        done.fetch_or(bit, std::memory_order_release);
+    }
+    return FP8ATTN_OK;
+}
 
 // ---------------------------------------------------------------------------- general kernel launch
 template <int D, int BN, int EB, int NPL, int MODE>
@@ -138,11 +190,8 @@ int launch_general(const CUtensorMap& mq, const CUtensorMap& mk, const CUtensorM
                    dim3 grid, cudaStream_t st) {
     using C = GeneralCfg<D, BN, EB, NPL, MODE>;
     auto kern = attn_general_kernel<D, BN, EB, NPL, MODE>;
-    static bool configured = false;
-    if (!configured) {
-        CU_TRY(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, C::SMEM_BYTES));
-        configured = true;
-    }
+    static std::atomic<unsigned long long> done{0};
+    if (int rc = ensure_smem(kern, C::SMEM_BYTES, done)) return rc;
     kern<<<grid, 128, C::SMEM_BYTES, st>>>(mq, mk, mv, p);
     CU_TRY(cudaGetLastError());
     return FP8ATTN_OK;
@@ -154,7 +203,7 @@ int dispatch_general(int d, int bn, const CUtensorMap& mq, const CUtensorMap& mk
     if constexpr (NPL == 3) {   // FP32 inputs: Bn = 64 only (three planes of Q, K, V must fit in shared memory)
         if (d == 64 && bn == 64) return launch_general<64, 64, EB, NPL, MODE>(mq, mk, mv, p, grid, st);
         if (d == 128 && bn == 64) return launch_general<128, 64, EB, NPL, MODE>(mq, mk, mv, p, grid, st);
-    } else if constexpr (EB == 1) {   // E4M3: d = 128 only
+    } else if constexpr (EB == 1) {   // E4M3: d = 128 only (a 64-byte operand row does not fill a 128-byte swizzle row)
         if (d == 128 && bn == 64) return launch_general<128, 64, EB, NPL, MODE>(mq, mk, mv, p, grid, st);
         if (d == 128 && bn == 128) return launch_general<128, 128, EB, NPL, MODE>(mq, mk, mv, p, grid, st);
     } else {
@@ -167,65 +216,29 @@ int dispatch_general(int d, int bn, const CUtensorMap& mq, const CUtensorMap& mk
     return FP8ATTN_E_UNSUPPORTED;
 }
 
-// ---------------------------------------------------------------------------- prefill kernel launch
-template <int EB, bool FOLD, int QKG>
-int launch_prefill_g(const CUtensorMap& mq, const CUtensorMap& mk, const CUtensorMap& mv, const FwdParams& p,
+// ---------------------------------------------------------------------------- prefill kernel launch (Bn = 128)
+template <int EB, bool FOLD>
+int launch_prefill(const CUtensorMap& mq, const CUtensorMap& mk, const CUtensorMap& mv, const FwdParams& p,
                    cudaStream_t st) {
-    using C = PrefillCfg<EB>;
-    auto kern = attn_prefill_kernel<EB, FOLD, QKG>;
-    static bool configured = false;
-    if (!configured) {
-        CU_TRY(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, C::SMEM_BYTES));
-        configured = true;
-    }
-    const dim3 grid((unsigned)((p.Lq + 2 * BM - 1) / (2 * BM)), (unsigned)(p.B * p.Hq));
-    kern<<<grid, C::THREADS, C::SMEM_BYTES, st>>>(mq, mk, mv, p);
-    CU_TRY(cudaGetLastError());
-    return FP8ATTN_OK;
-}
-
-// ---------------------------------------------------------------------------- prefill kernel, third structure
-template <int EB, bool FOLD>
-int launch_prefill3(const CUtensorMap& mq, const CUtensorMap& mk, const CUtensorMap& mv, const FwdParams& p,
-                    cudaStream_t st) {
-    using C = Prefill3Cfg<EB>;
-    auto kern = attn_prefill3_kernel<EB, FOLD>;
-    static const int alternate = [] {
-        const char* e = getenv("FP8ATTN_ALT");
-        return e ? atoi(e) : 0;
-    }();
-    FwdParams pa = p;
-    pa.alternate = alternate;
-    static bool configured = false;
-    if (!configured) {
-        CU_TRY(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, C::SMEM_BYTES));
-        configured = true;
-    }
-    const dim3 grid((unsigned)((p.Lq + 2 * BM - 1) / (2 * BM)), (unsigned)(p.B * p.Hq));
-    kern<<<grid, C::THREADS, C::SMEM_BYTES, st>>>(mq, mk, mv, pa);
-    CU_TRY(cudaGetLastError());
-    return FP8ATTN_OK;
-}
-
-// ---------------------------------------------------------------------------- prefill kernel, fourth structure
-template <int EB, bool FOLD>
-int launch_prefill4(const CUtensorMap& mq, const CUtensorMap& mk, const CUtensorMap& mv, const FwdParams& p,
-                    cudaStream_t st) {
-    using C = Prefill4Cfg<EB>;
+    using C = PrefillKCfg<EB>;
     // the statistics instance (P dump, underflow counters of fp8attn_stats) has the same schedule; the plain
     // instance carries none of that code
-    const int aux = (p.p_codes || p.underflow) ? 1 : 0;
-    auto kern = aux ? attn_prefill4_kernel<EB, FOLD, true> : attn_prefill4_kernel<EB, FOLD, false>;
-    static bool configured[2] = {false, false};
-    if (!configured[aux]) {
-        CU_TRY(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, C::SMEM_BYTES));
-        configured[aux] = true;
-    }
+    const bool aux = p.p_codes || p.underflow;
     // o as [B*Hq, Lq, d] FP32: boxes of 32 rows x 32 floats, stored by TMA from the epilogue
     CUtensorMap mo;
     if (int rc = make_map(&mo, p.o, 4, (long long)p.B * p.Hq, p.Lq, 128, 32)) return rc;
     const dim3 grid((unsigned)(((p.Lq + 2 * BM - 1) / (2 * BM)) * (p.B * p.Hq)));
-    kern<<<grid, C::THREADS, C::SMEM_BYTES, st>>>(mq, mk, mv, mo, p);
+    if (aux) {
+        auto kern = attn_prefill_kernel<EB, FOLD, true>;
+        static std::atomic<unsigned long long> done{0};
+        if (int rc = ensure_smem(kern, C::SMEM_BYTES, done)) return rc;
+        kern<<<grid, C::THREADS, C::SMEM_BYTES, st>>>(mq, mk, mv, mo, p);
+    } else {
+        auto kern = attn_prefill_kernel<EB, FOLD, false>;
+        static std::atomic<unsigned long long> done{0};
+        if (int rc = ensure_smem(kern, C::SMEM_BYTES, done)) return rc;
+        kern<<<grid, C::THREADS, C::SMEM_BYTES, st>>>(mq, mk, mv, mo, p);
+    }
     CU_TRY(cudaGetLastError());
     return FP8ATTN_OK;
 }
@@ -235,28 +248,30 @@ template <int EB, bool FOLD>
 int launch_prefill64(const CUtensorMap& mq, const CUtensorMap& mk, const CUtensorMap& mv, const FwdParams& p,
                      cudaStream_t st) {
     using C = Prefill64Cfg<EB>;
-    auto kern = attn_prefill64_kernel<EB, FOLD>;
-    static bool configured = false;
-    if (!configured) {
-        CU_TRY(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, C::SMEM_BYTES));
-        configured = true;
+    const bool aux = p.p_codes || p.underflow;
+    const dim3 grid((unsigned)(((p.Lq + 2 * BM - 1) / (2 * BM)) * (p.B * p.Hq)));
+    if (aux) {
+        auto kern = attn_prefill64_kernel<EB, FOLD, true>;
+        static std::atomic<unsigned long long> done{0};
+        if (int rc = ensure_smem(kern, C::SMEM_BYTES, done)) return rc;
+        kern<<<grid, C::THREADS, C::SMEM_BYTES, st>>>(mq, mk, mv, p);
+    } else {
+        auto kern = attn_prefill64_kernel<EB, FOLD, false>;
+        static std::atomic<unsigned long long> done{0};
+        if (int rc = ensure_smem(kern, C::SMEM_BYTES, done)) return rc;
+        kern<<<grid, C::THREADS, C::SMEM_BYTES, st>>>(mq, mk, mv, p);
     }
-    const dim3 grid((unsigned)((p.Lq + 2 * BM - 1) / (2 * BM)), (unsigned)(p.B * p.Hq));
-    kern<<<grid, C::THREADS, C::SMEM_BYTES, st>>>(mq, mk, mv, p);
     CU_TRY(cudaGetLastError());
     return FP8ATTN_OK;
 }
 
 // ---------------------------------------------------------------------------- decode kernel launch
-template <int NVT, bool FOLD>
+template <int NVT, bool FOLD, bool AUX>
 int launch_decode_t(const CUtensorMap& mq, const CUtensorMap& mk, const CUtensorMap& mv, const FwdParams& p,
                     cudaStream_t st) {
-    auto kern = attn_decode_kernel<NVT, FOLD>;
-    static bool configured = false;
-    if (!configured) {
-        CU_TRY(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, DecodeCfg::SMEM_BYTES));
-        configured = true;
-    }
+    auto kern = attn_decode_kernel<NVT, FOLD, AUX>;
+    static std::atomic<unsigned long long> done{0};
+    if (int rc = ensure_smem(kern, DecodeCfg::SMEM_BYTES, done)) return rc;
     const dim3 grid((unsigned)(p.B * p.Hkv), (unsigned)p.num_splits);
     kern<<<grid, DecodeCfg::THREADS, DecodeCfg::SMEM_BYTES, st>>>(mq, mk, mv, p);
     CU_TRY(cudaGetLastError());
@@ -265,9 +280,15 @@ int launch_decode_t(const CUtensorMap& mq, const CUtensorMap& mk, const CUtensor
 template <bool FOLD>
 int launch_decode(int nv, const CUtensorMap& mq, const CUtensorMap& mk, const CUtensorMap& mv, const FwdParams& p,
                   cudaStream_t st) {
-    if (nv <= 4) return launch_decode_t<4, FOLD>(mq, mk, mv, p, st);
-    if (nv <= 8) return launch_decode_t<8, FOLD>(mq, mk, mv, p, st);
-    return launch_decode_t<16, FOLD>(mq, mk, mv, p, st);
+    // the statistics instance (P dump, underflow counters) has the same schedule; the plain one carries no such code
+    if (p.p_codes || p.underflow) {
+        if (nv <= 4) return launch_decode_t<4, FOLD, true>(mq, mk, mv, p, st);
+        if (nv <= 8) return launch_decode_t<8, FOLD, true>(mq, mk, mv, p, st);
+        return launch_decode_t<16, FOLD, true>(mq, mk, mv, p, st);
+    }
+    if (nv <= 4) return launch_decode_t<4, FOLD, false>(mq, mk, mv, p, st);
+    if (nv <= 8) return launch_decode_t<8, FOLD, false>(mq, mk, mv, p, st);
+    return launch_decode_t<16, FOLD, false>(mq, mk, mv, p, st);
 }
 // Number of KV splits for the decode kernel: enough CTAs to fill 2 x 148 resident slots several times over,
 // with a last wave that is nearly full.
@@ -282,32 +303,6 @@ int decode_auto_splits(long long kv_slabs, int nb) {
         if (nb / ns < 8) break;      // keep at least 8 blocks per split
     }
     return best;
-}
-
-int prefill_variant() {
-    static const int variant = [] {
-        const char* e = getenv("FP8ATTN_PREFILL_V");
-        return e ? atoi(e) : 4;
-    }();
-    return variant;
-}
-// Bn = 128 prefill kernels.  FP8ATTN_PREFILL_V selects the structure (4, the default: attn_prefill4.cuh; 3:
-// attn_prefill3.cuh; 1: attn_prefill.cuh, whose QK^T issue granularity FP8ATTN_QKG = 1, 2 or 4 sets).  These are
-// development / cross-check knobs, read once per process: every structure computes the same Alg. 1 values.
-template <int EB, bool FOLD>
-int launch_prefill(const CUtensorMap& mq, const CUtensorMap& mk, const CUtensorMap& mv, const FwdParams& p,
-                   cudaStream_t st) {
-    static const int qkg = [] {
-        const char* e = getenv("FP8ATTN_QKG");
-        const int v = e ? atoi(e) : 0;
-        return (v == 1 || v == 2 || v == 4) ? v : 2;
-    }();
-    const int variant = prefill_variant();
-    if (variant == 4) return launch_prefill4<EB, FOLD>(mq, mk, mv, p, st);
-    if (variant == 3) return launch_prefill3<EB, FOLD>(mq, mk, mv, p, st);
-    if (qkg == 1) return launch_prefill_g<EB, FOLD, 1>(mq, mk, mv, p, st);
-    if (qkg == 4) return launch_prefill_g<EB, FOLD, 4>(mq, mk, mv, p, st);
-    return launch_prefill_g<EB, FOLD, 2>(mq, mk, mv, p, st);
 }
 
 // S = 2^k with a comfortable exponent: the factor can be folded into the exponent of P exactly
@@ -342,7 +337,7 @@ int validate_args(const void* q, const void* k, const void* v, const void* o, in
     if (stats && (stats->kernel < 0 || stats->kernel > 3 || stats->reserved0 != 0)) return FP8ATTN_E_MODE;
     if (stats && stats->p_codes && (stats->p_batch < 0 || stats->p_batch >= B || stats->p_head < 0 || stats->p_head >= Hq))
         return FP8ATTN_E_SHAPE;
-    if ((long long)B * Hq > 65535) return FP8ATTN_E_UNSUPPORTED;
+    if ((long long)B * Hq * ((Lq + 127) / 128) > 0x7FFFFFFFll) return FP8ATTN_E_UNSUPPORTED;
     return FP8ATTN_OK;
 }
 
@@ -353,7 +348,16 @@ int validate_args(const void* q, const void* k, const void* v, const void* o, in
 // =============================================================================================
 extern "C" {
 
-int fp8attn_version(void) { return 100; }   // 0.1.0
+int fp8attn_version(void) { return 200; }   // 0.2.0
+
+int fp8attn_trim(void) {
+    int dev = 0;
+    if (int rc = current_device(&dev)) return rc;
+    DeviceState& d = g_dev[dev];
+    std::lock_guard<std::mutex> lock(d.mu);
+    if (d.pool) CU_TRY(cudaMemPoolTrimTo(d.pool, 0));
+    return FP8ATTN_OK;
+}
 
 const char* fp8attn_last_cuda_error(void) { return g_err; }
 
@@ -385,12 +389,13 @@ int fp8attn_fwd(const void* q, const void* k, const void* v, void* o, int B, int
     cudaStream_t st = stats ? reinterpret_cast<cudaStream_t>(stats->stream) : nullptr;
     const int nb = (Lk + bn - 1) / bn;
     const int n_qtiles = (Lq + BM - 1) / BM;
-    const int want_kernel_early = stats ? stats->kernel : 0;
-    const bool decode_shape = pm == 2 && d == 128 && bn == 128 && (long long)(Hq / Hkv) * Lq <= 16 &&
-                              !(stats && (stats->p_codes || stats->underflow));
-    if (ns == 0 && decode_shape && want_kernel_early != 1 && want_kernel_early != 2) {
-        ns = decode_auto_splits(kv_slabs, nb);
-    }
+    const int want_kernel = stats ? stats->kernel : 0;
+    const bool want_aux = stats && (stats->p_codes || stats->underflow);
+    // decode shape: a handful of query rows per kv head against an E4M3 KV cache
+    const bool decode_ok = pm == 2 && d == 128 && bn == 128 && (long long)(Hq / Hkv) * Lq <= 16;
+    if (want_kernel == 3 && !decode_ok) return FP8ATTN_E_UNSUPPORTED;
+    const bool use_decode = decode_ok && (want_kernel == 3 || want_kernel == 0);
+    if (ns == 0 && use_decode) ns = decode_auto_splits(kv_slabs, nb);
     if (ns == 0) {
         // automatic: split only decode-shaped calls (a handful of query rows per head) whose query
         // tiles alone cannot fill the GPU.  Splitting changes which P values are cast against the
@@ -405,17 +410,16 @@ int fp8attn_fwd(const void* q, const void* k, const void* v, void* o, int B, int
     }
     if (ns > nb) ns = nb;
 
-    std::lock_guard<std::mutex> lock(g_mu);
     const long long nq = q_slabs * Lq * d, nkv = kv_slabs * Lk * d;
     const void *qs = q, *ks = k, *vs = v;   // staged operands the kernel reads
     const float* q_scale = stats ? stats->q_scale : nullptr;
     int n_launches = 0;
     int eb = 2, npl = 1;
+    Lease planes, qquant, amax_buf, partial;     // per-call scratch, returned to the pool on `st` at return
     if (dt == 0) {
         // FP32 -> three BF16 planes each (exact split), so that tcgen05 reproduces FP32 logits
-        void* ws = nullptr;
-        if (int rc = g_planes.get(&ws, (size_t)(nq + 2 * nkv) * 3 * 2, st)) return rc;
-        uint16_t* pq = static_cast<uint16_t*>(ws);
+        if (int rc = planes.get((size_t)(nq + 2 * nkv) * 3 * 2, st)) return rc;
+        uint16_t* pq = static_cast<uint16_t*>(planes.ptr);
         uint16_t* pk = pq + 3 * nq;
         uint16_t* pv = pk + 3 * nkv;
         const int thr = 256;
@@ -432,12 +436,9 @@ int fp8attn_fwd(const void* q, const void* k, const void* v, void* o, int B, int
     } else if (dt == 3) {
         // decode: quantise the BF16 q of every (b, hq) slab to E4M3 (reading R24 in DESIGN.md)
         eb = 1;
-        void *wq = nullptr, *wa = nullptr;
-        if (int rc = g_qquant.get(&wq, (size_t)nq + (size_t)q_slabs * 4 + 16, st)) return rc;
-        if (int rc = g_amax.get(&wa, (size_t)q_slabs * 4, st)) return rc;
-        uint8_t* codes = static_cast<uint8_t*>(wq);
+        if (int rc = qquant.get((size_t)nq + (size_t)q_slabs * 4 + 16, st)) return rc;
+        uint8_t* codes = static_cast<uint8_t*>(qquant.ptr);
         float* qsc = reinterpret_cast<float*>(codes + ((nq + 15) / 16) * 16);
-        unsigned int* amax = static_cast<unsigned int*>(wa);
         const long long slab = (long long)Lq * d;
         if (slab <= 4096) {
             // a decode-sized q: one warp per slab does absmax, codes and scale in one launch
@@ -446,11 +447,13 @@ int fp8attn_fwd(const void* q, const void* k, const void* v, void* o, int B, int
             CU_TRY(cudaGetLastError());
             n_launches += 1;
         } else {
+            if (int rc = amax_buf.get((size_t)q_slabs * 4, st)) return rc;
+            unsigned int* amax = static_cast<unsigned int*>(amax_buf.ptr);
             CU_TRY(cudaMemsetAsync(amax, 0, (size_t)q_slabs * 4, st));
-            unsigned gx = (unsigned)((slab + 255) / 256);
-            if (gx > 64) gx = 64;
-            absmax_kernel<__nv_bfloat16><<<dim3(gx, (unsigned)q_slabs), 256, 0, st>>>(static_cast<const __nv_bfloat16*>(q), amax, slab);
-            quantize_kernel<__nv_bfloat16><<<dim3(gx, (unsigned)q_slabs), 256, 0, st>>>(static_cast<const __nv_bfloat16*>(q), amax, codes, slab);
+            unsigned gy = (unsigned)((slab + 255) / 256);
+            if (gy > 64) gy = 64;
+            absmax_kernel<__nv_bfloat16><<<dim3((unsigned)q_slabs, gy), 256, 0, st>>>(static_cast<const __nv_bfloat16*>(q), amax, slab);
+            quantize_kernel<__nv_bfloat16><<<dim3((unsigned)q_slabs, gy), 256, 0, st>>>(static_cast<const __nv_bfloat16*>(q), amax, codes, slab);
             finalize_scale_kernel<<<(unsigned)((q_slabs + 255) / 256), 256, 0, st>>>(amax, qsc, (int)q_slabs);
             CU_TRY(cudaGetLastError());
             n_launches += 3;
@@ -487,28 +490,26 @@ int fp8attn_fwd(const void* q, const void* k, const void* v, void* o, int B, int
     p.sm_scale = 1.0f / sqrtf((float)d);
     const long long R = q_slabs * Lq;
     if (ns > 1) {
-        void* ws = nullptr;
-        if (int rc = g_partial.get(&ws, (size_t)ns * R * (d + 2) * 4, st)) return rc;
-        p.part_o = static_cast<float*>(ws);
+        if (int rc = partial.get((size_t)ns * R * (d + 2) * 4, st)) return rc;
+        p.part_o = static_cast<float*>(partial.ptr);
         p.part_ml = p.part_o + (size_t)ns * R * d;
     }
+    if (pm == 0) p.p_codes = nullptr;          // the no-cast mode has no codes (and counts nothing)
     if (p.underflow) CU_TRY(cudaMemsetAsync(p.underflow, 0, 2 * sizeof(unsigned long long), st));
+    // masked positions of the P dump (and the blocks a causal tile skips) read 0xFF
+    if (p.p_codes) CU_TRY(cudaMemsetAsync(p.p_codes, 0xFF, (size_t)Lq * Lk, st));
 
-    // kernel family: the warp-specialised prefill kernel serves d = 128, Bn = 128, one split, BF16 or
-    // E4M3 operands, modes 1 and 2, when neither the P dump nor the underflow counters are asked for.
-    const int want_kernel = stats ? stats->kernel : 0;
-    const bool prefill_ok = d == 128 && (bn == 128 || bn == 64) && ns == 1 && npl == 1 && pm != 0 && dt != 3 &&
-                            ((!p.p_codes && !p.underflow) || (bn == 128 && prefill_variant() == 4));
+    // kernel family.  The warp-specialised prefill kernels serve d = 128, one split, BF16 or E4M3 operands,
+    // modes 1 and 2 (Bn = 128 and Bn = 64); the decode kernel serves decode shapes with any split count; each
+    // has a statistics instance (same schedule + P dump + underflow counters).  Everything else -- FP32
+    // inputs, the no-cast mode, d = 64, prefill with splits -- runs on the general kernel.
+    const bool prefill_ok = d == 128 && ns == 1 && npl == 1 && pm != 0 && dt != 3;
     if (want_kernel == 2 && !prefill_ok) return FP8ATTN_E_UNSUPPORTED;
-    const bool decode_ok = decode_shape && eb == 1 && npl == 1;
-    if (want_kernel == 3 && !decode_ok) return FP8ATTN_E_UNSUPPORTED;
-    const bool use_decode = decode_ok && (want_kernel == 3 || want_kernel == 0);
-    // (automatic selection keeps calls that ask for the P dump or the underflow counters on the general kernel;
-    // the statistics instance of the prefill kernel serves them on request, stats->kernel = 2)
-    const bool use_prefill = !use_decode && prefill_ok &&
-                             (want_kernel == 2 || (want_kernel == 0 && Lq > 16 && !p.p_codes && !p.underflow));
+    // (automatic selection keeps prefill-shaped calls that ask for the P dump or the underflow counters on the
+    // general kernel, whose serial schedule is the reference for them; stats->kernel = 2 takes the statistics
+    // instance of the throughput kernel)
+    const bool use_prefill = !use_decode && prefill_ok && (want_kernel == 2 || (want_kernel == 0 && Lq > 16 && !want_aux));
     int kernel_id = 1;
-    const dim3 grid((unsigned)n_qtiles, (unsigned)q_slabs, (unsigned)ns);
     int rc;
     if (use_decode) {
         kernel_id = 3;
@@ -525,14 +526,17 @@ int fp8attn_fwd(const void* q, const void* k, const void* v, void* o, int B, int
             else rc = fold ? launch_prefill64<2, true>(mq, mk, mv, p, st) : launch_prefill64<2, false>(mq, mk, mv, p, st);
         } else if (eb == 1) rc = fold ? launch_prefill<1, true>(mq, mk, mv, p, st) : launch_prefill<1, false>(mq, mk, mv, p, st);
         else rc = fold ? launch_prefill<2, true>(mq, mk, mv, p, st) : launch_prefill<2, false>(mq, mk, mv, p, st);
-    } else if (npl == 3)
-        rc = (pm == 0) ? dispatch_general<2, 3, 0>(d, bn, mq, mk, mv, p, grid, st)
-                       : dispatch_general<2, 3, 1>(d, bn, mq, mk, mv, p, grid, st);
-    else if (eb == 2)
-        rc = (pm == 0) ? dispatch_general<2, 1, 0>(d, bn, mq, mk, mv, p, grid, st)
-                       : dispatch_general<2, 1, 1>(d, bn, mq, mk, mv, p, grid, st);
-    else
-        rc = dispatch_general<1, 1, 2>(d, bn, mq, mk, mv, p, grid, st);
+    } else {
+        const dim3 grid((unsigned)(n_qtiles * q_slabs), 1u, (unsigned)ns);
+        if (npl == 3)
+            rc = (pm == 0) ? dispatch_general<2, 3, 0>(d, bn, mq, mk, mv, p, grid, st)
+                           : dispatch_general<2, 3, 1>(d, bn, mq, mk, mv, p, grid, st);
+        else if (eb == 2)
+            rc = (pm == 0) ? dispatch_general<2, 1, 0>(d, bn, mq, mk, mv, p, grid, st)
+                           : dispatch_general<2, 1, 1>(d, bn, mq, mk, mv, p, grid, st);
+        else
+            rc = dispatch_general<1, 1, 2>(d, bn, mq, mk, mv, p, grid, st);
+    }
     if (rc) return rc;
     ++n_launches;
     if (ns > 1) {
@@ -580,12 +584,23 @@ int fp8attn_fwd_host(const void* q, const void* k, const void* v, void* o, int B
     const size_t o_pc = off;  off += (stats && stats->p_codes) ? up((size_t)Lq * Lk) : 0;
 
     cudaStream_t st = stats ? reinterpret_cast<cudaStream_t>(stats->stream) : nullptr;
-    static std::mutex host_mu;
-    static Scratch host_buf;
-    std::lock_guard<std::mutex> lock(host_mu);
-    void* ws = nullptr;
-    if (int rc = host_buf.get(&ws, off, st)) return rc;
-    uint8_t* base = static_cast<uint8_t*>(ws);
+    int dev_now = 0;
+    if (int rc = current_device(&dev_now)) return rc;
+    DeviceState& ds_dev = g_dev[dev_now];
+    std::lock_guard<std::mutex> lock(ds_dev.host_mu);
+    Lease staging;                      // returned to the pool after the final synchronisation below
+    if (int rc = staging.get(off, st)) return rc;
+    // whatever way this function is left, no copy may still be in flight when the staging memory goes back
+    struct Drain {
+        DeviceState& d;
+        cudaStream_t st;
+        ~Drain() {
+            if (d.s_in) cudaStreamSynchronize(d.s_in);
+            cudaStreamSynchronize(st);
+            if (d.s_out) cudaStreamSynchronize(d.s_out);
+        }
+    } drain{ds_dev, st};
+    uint8_t* base = static_cast<uint8_t*>(staging.ptr);
     fp8attn_stats dstats;
     fp8attn_stats* ds = nullptr;
     if (stats) {
@@ -608,7 +623,6 @@ int fp8attn_fwd_host(const void* q, const void* k, const void* v, void* o, int B
         if (stats->underflow) dstats.underflow = reinterpret_cast<unsigned long long*>(base + o_uf);
         if (stats->p_codes) {
             dstats.p_codes = base + o_pc;
-            CU_TRY(cudaMemsetAsync(base + o_pc, 0xFF, (size_t)Lq * Lk, st));
         }
     }
     // (batch, kv-head group) slabs are independent and contiguous in q, k, v and o: large
@@ -622,10 +636,11 @@ int fp8attn_fwd_host(const void* q, const void* k, const void* v, void* o, int B
     const bool auto_split = (long long)(Hq / Hkv) * Lq <= 16 && !(stats && stats->num_splits > 0);
     if (traffic >= (size_t(32) << 20) && !auto_split && !(stats && (stats->p_codes || stats->underflow))) {
         pieces_b = B < 8 ? B : 8;
-        while (pieces_b * pieces_h < 8 && Hkv % (pieces_h * 2) == 0) pieces_h *= 2;
-        if (B >= 8) pieces_h = 1;
+        // pieces along the kv heads: the largest power of two that divides Hkv and keeps the total at 8 or less
+        while (pieces_b * pieces_h * 2 <= 8 && Hkv % (pieces_h * 2) == 0) pieces_h *= 2;
     }
-    const int n_pieces = pieces_b * pieces_h;
+    const int n_pieces = pieces_b * pieces_h;      // <= 8: the size of the event arrays
+    if (n_pieces > 8) return FP8ATTN_E_UNSUPPORTED;
     if (n_pieces == 1) {
         CU_TRY(cudaMemcpyAsync(base + o_q, q, nq * ebq, cudaMemcpyHostToDevice, st));
         CU_TRY(cudaMemcpyAsync(base + o_k, k, nkv * ebkv, cudaMemcpyHostToDevice, st));
@@ -642,23 +657,13 @@ int fp8attn_fwd_host(const void* q, const void* k, const void* v, void* o, int B
                 CU_TRY(cudaMemcpyAsync(stats->p_codes, base + o_pc, (size_t)Lq * Lk, cudaMemcpyDeviceToHost, st));
         }
     } else {
-        static cudaStream_t s_in = nullptr, s_out = nullptr;
-        static cudaEvent_t ev_start = nullptr, ev_in[8], ev_done[8];
-        static int s_dev = -1;
-        int dev_now = 0;
-        cudaGetDevice(&dev_now);
-        if (s_in && s_dev != dev_now) {      // streams and events belong to the device they were created on
-            cudaStreamDestroy(s_in);
-            cudaStreamDestroy(s_out);
-            cudaEventDestroy(ev_start);
-            for (int i = 0; i < 8; ++i) {
-                cudaEventDestroy(ev_in[i]);
-                cudaEventDestroy(ev_done[i]);
-            }
-            s_in = nullptr;
-        }
+        // the copy streams and events of this device, created on first use
+        cudaStream_t& s_in = ds_dev.s_in;
+        cudaStream_t& s_out = ds_dev.s_out;
+        cudaEvent_t& ev_start = ds_dev.ev_start;
+        cudaEvent_t* const ev_in = ds_dev.ev_in;
+        cudaEvent_t* const ev_done = ds_dev.ev_done;
         if (!s_in) {
-            s_dev = dev_now;
             CU_TRY(cudaStreamCreateWithFlags(&s_in, cudaStreamNonBlocking));
             CU_TRY(cudaStreamCreateWithFlags(&s_out, cudaStreamNonBlocking));
             CU_TRY(cudaEventCreateWithFlags(&ev_start, cudaEventDisableTiming));
@@ -742,16 +747,15 @@ int fp8attn_quantize_e4m3(const float* x, uint8_t* out_codes, float* out_scale, 
     if (int rc = check_device()) return rc;
     cudaStream_t st = reinterpret_cast<cudaStream_t>(stream);
     const long long slabs = (long long)B * H, slab = (long long)L * d;
-    if (slabs > 65535) return FP8ATTN_E_UNSUPPORTED;
-    std::lock_guard<std::mutex> lock(g_mu);
-    void* wa = nullptr;
-    if (int rc = g_amax.get(&wa, (size_t)slabs * 4, st)) return rc;
-    unsigned int* amax = static_cast<unsigned int*>(wa);
+    if (slabs > 0x7FFFFFFFll) return FP8ATTN_E_UNSUPPORTED;
+    Lease amax_buf;
+    if (int rc = amax_buf.get((size_t)slabs * 4, st)) return rc;
+    unsigned int* amax = static_cast<unsigned int*>(amax_buf.ptr);
     CU_TRY(cudaMemsetAsync(amax, 0, (size_t)slabs * 4, st));
-    unsigned gx = (unsigned)((slab + 1023) / 1024);
-    if (gx > 148) gx = 148;
-    absmax_kernel<float><<<dim3(gx, (unsigned)slabs), 256, 0, st>>>(x, amax, slab);
-    quantize_kernel<float><<<dim3(gx, (unsigned)slabs), 256, 0, st>>>(x, amax, out_codes, slab);
+    unsigned gy = (unsigned)((slab + 1023) / 1024);
+    if (gy > 148) gy = 148;
+    absmax_kernel<float><<<dim3((unsigned)slabs, gy), 256, 0, st>>>(x, amax, slab);
+    quantize_kernel<float><<<dim3((unsigned)slabs, gy), 256, 0, st>>>(x, amax, out_codes, slab);
     finalize_scale_kernel<<<(unsigned)((slabs + 255) / 256), 256, 0, st>>>(amax, out_scale, (int)slabs);
     CU_TRY(cudaGetLastError());
     return FP8ATTN_OK;
@@ -786,15 +790,3 @@ int fp8attn_debug_gemm(const void* A, const void* Bm, float* D, int N, int K, in
 }
 
 }  // extern "C"
-
-#ifdef FP8ATTN_TRACE
-// development build only: copies the clock64 stamps of attn_prefill3_kernel to the host
-extern "C" __attribute__((visibility("default"))) int fp8attn_debug_trace(long long* out, int n) {
-    if (n > 2 * 80 * 16) n = 2 * 80 * 16;
-    return (int)cudaMemcpyFromSymbol(out, fp8attn::g_trace3, (size_t)n * sizeof(long long));
-}
-extern "C" __attribute__((visibility("default"))) int fp8attn_debug_trace4(long long* out, int n) {
-    if (n > 4096 * 8) n = 4096 * 8;
-    return (int)cudaMemcpyFromSymbol(out, fp8attn::g_trace4, (size_t)n * sizeof(long long));
-}
-#endif

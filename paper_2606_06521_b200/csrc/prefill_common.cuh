@@ -1,0 +1,184 @@
+// prefill_common.cuh -- building blocks shared by the warp-specialised prefill kernels (attn_prefill.cuh, Bn = 128;
+// attn_prefill64.cuh, Bn = 64): operand geometry, the exp / sum / cast pass of Alg. 1 lines 7-9
+// on one 32-column chunk, the FMA-pipe exp2, row max / mask helpers, the P hand-off and the O rescale warp.
+#pragma once
+#include "common.cuh"
+
+namespace fp8attn {
+
+template <int EB>
+struct PrefillCfg {
+    static constexpr int D = 128, BN = 128;
+    static constexpr int CH = 128 / EB;              // elements per 128-byte swizzle row
+    static constexpr int NCH = D / CH;               // 128-byte chunks per operand row
+    static constexpr int TILE = NCH * 128 * 128;     // bytes of one 128-row operand tile (Q, K_j or V_j)
+    static constexpr int NS = (EB == 1) ? 4 : 2;     // K ring depth = V ring depth
+    static constexpr int KSTEP = 32 / EB;            // contraction elements per MMA
+    static constexpr int P_COLS = BN * EB / 4;       // TMEM columns of P
+    static constexpr int TM_S = 0, TM_O = 256;
+    static constexpr uint32_t KIND = (EB == 1) ? ptx::KIND_F8F6F4 : ptx::KIND_F16;
+    static constexpr uint32_t FMT = (EB == 1) ? ptx::FMT_E4M3 : ptx::FMT_BF16;
+};
+
+// exact E4M3 pair -> BF16 pair: the code shifted left by 4 is the BF16 bit pattern of value * 2^-120
+// (subnormal codes map to BF16 subnormals), and the packed multiply by 2^120 is exact.
+__device__ __forceinline__ uint32_t e4m3x2_to_bf16x2(uint32_t pair) {
+    const uint32_t spread = ((pair & 0xFF00u) << 12) | ((pair & 0xFFu) << 4);
+    uint32_t r;
+    asm("mul.rn.bf16x2 %0, %1, %2;" : "=r"(r) : "r"(spread), "r"(0x7B807B80u));   // 2^120 in both halves
+    return r;
+}
+
+// 2^x for a packed pair on the FMA pipe (the MUFU pipe is the busy one in the exp pass): x = n + f with
+// n = round(x) taken from the low mantissa bits of x + 1.5 * 2^23, f in [-0.5, 0.5], a degree-5 polynomial for
+// 2^f (near-minimax, Chebyshev nodes; max relative error 2.3e-7 in FP32 Horner form, the same order as
+// ex2.approx), and n added to the exponent field.  x is clamped at -125 (2^-125 casts to E4M3 zero and adds
+// nothing to a row sum that holds at least one term equal to S).
+__device__ __forceinline__ void exp2_poly2(uint64_t x2, float& r0, float& r1) {
+    constexpr float MAGIC = 12582912.0f;
+    float x0, x1;
+    ptx::unpack2(x2, x0, x1);
+    x0 = fmaxf(x0, -125.0f);
+    x1 = fmaxf(x1, -125.0f);
+    const uint64_t xc = ptx::pack2(x0, x1);
+    const uint64_t t2 = ptx::add2(xc, ptx::pack2(MAGIC, MAGIC));
+    const uint64_t n2 = ptx::add2(t2, ptx::pack2(-MAGIC, -MAGIC));
+    const uint64_t f2 = ptx::fma2(n2, ptx::pack2(-1.0f, -1.0f), xc);
+    uint64_t p2 = ptx::fma2(ptx::pack2(0.00134004f, 0.00134004f), f2, ptx::pack2(0.00967604f, 0.00967604f));
+    p2 = ptx::fma2(p2, f2, ptx::pack2(0.05550327f, 0.05550327f));
+    p2 = ptx::fma2(p2, f2, ptx::pack2(0.24022107f, 0.24022107f));
+    p2 = ptx::fma2(p2, f2, ptx::pack2(0.6931472f, 0.6931472f));
+    p2 = ptx::fma2(p2, f2, ptx::pack2(1.0000001f, 1.0000001f));
+    float p0, p1, t0, t1;
+    ptx::unpack2(p2, p0, p1);
+    ptx::unpack2(t2, t0, t1);
+    r0 = __int_as_float(__float_as_int(p0) + (__float_as_int(t0) << 23));
+    r1 = __int_as_float(__float_as_int(p1) + (__float_as_int(t1) << 23));
+}
+
+// ---- one 32-column chunk of the exp pass (Alg. 1 lines 7-9) -------------------------------------
+// v: raw logits of 32 keys.  Returns P codes / BF16 values in w (P_COLS/4 words) and adds the FP32
+// pre-cast P (times S when the scale is folded into the exponent) to the two packed sums.
+// NPOLY: bit i set = element pair i of the 16 pairs of the chunk takes exp2_poly2 instead of ex2.approx
+// (0: all on the MUFU pipe).
+template <int EB, bool FOLD, bool MASK, int NPOLY = 0>
+__device__ __forceinline__ void exp_chunk(const uint32_t* v, uint32_t* w, int j_first, int jlim, uint64_t cl2_2,
+                                          uint64_t negm_2, uint64_t s_2, uint64_t& sum_a, uint64_t& sum_b) {
+    float pr[32];
+#pragma unroll
+    for (int e = 0; e < 32; e += 2) {
+        uint32_t a = v[e], b = v[e + 1];
+        if constexpr (MASK) {
+            if (j_first + e > jlim) a = 0xFF800000u;       // -inf
+            if (j_first + e + 1 > jlim) b = 0xFF800000u;
+        }
+        const uint64_t x = ptx::fma2(ptx::pack2u(a, b), cl2_2, negm_2);
+        if ((NPOLY >> (e >> 1)) & 1) {
+            exp2_poly2(x, pr[e], pr[e + 1]);
+        } else {
+            float x0, x1;
+            ptx::unpack2(x, x0, x1);
+            pr[e] = ptx::ex2_approx(x0);
+            pr[e + 1] = ptx::ex2_approx(x1);
+        }
+    }
+    uint32_t pair[16];
+#pragma unroll
+    for (int e = 0; e < 32; e += 4) {
+        const uint64_t p0 = ptx::pack2(pr[e], pr[e + 1]), p1 = ptx::pack2(pr[e + 2], pr[e + 3]);
+        sum_a = ptx::add2(sum_a, p0);
+        sum_b = ptx::add2(sum_b, p1);
+    }
+    if constexpr (!FOLD) {
+#pragma unroll
+        for (int e = 0; e < 32; e += 2) {
+            float y0, y1;
+            ptx::unpack2(ptx::mul2(ptx::pack2(pr[e], pr[e + 1]), s_2), y0, y1);
+            pair[e / 2] = ptx::cvt_e4m3x2(y0, y1);
+        }
+    } else {
+#pragma unroll
+        for (int e = 0; e < 32; e += 2) pair[e / 2] = ptx::cvt_e4m3x2(pr[e], pr[e + 1]);
+    }
+    if constexpr (EB == 1) {
+#pragma unroll
+        for (int e = 0; e < 8; ++e) w[e] = pair[2 * e] | (pair[2 * e + 1] << 16);
+    } else {
+#pragma unroll
+        for (int e = 0; e < 16; ++e) w[e] = e4m3x2_to_bf16x2(pair[e]);
+    }
+}
+
+// max over 32 (masked) raw logits folded into m
+__device__ __forceinline__ float max32(const uint32_t* v, float m) {
+    float m0 = m, m1 = -INFINITY;
+#pragma unroll
+    for (int e = 0; e < 32; e += 4) {
+        m0 = fmaxf(fmaxf(m0, __uint_as_float(v[e])), __uint_as_float(v[e + 1]));
+        m1 = fmaxf(fmaxf(m1, __uint_as_float(v[e + 2])), __uint_as_float(v[e + 3]));
+    }
+    return fmaxf(m0, m1);
+}
+__device__ __forceinline__ void mask32(uint32_t* v, int j_first, int jlim) {
+#pragma unroll
+    for (int e = 0; e < 32; ++e)
+        if (j_first + e > jlim) v[e] = 0xFF800000u;   // -inf
+}
+
+
+// Statistics of one 32-key chunk of P (statistics instances only): the E4M3 codes of the visible keys go to
+// dump_row (this query row of the P dump of fp8attn_stats, or null) and the zero codes among the visible
+// non-sink keys are counted into *uf (Prop. 1; null = not counted).  w holds the chunk as
+// exp_chunk leaves it; BF16 mode recovers a code from its exact BF16 value: times 2^-120, shifted right by 4.
+template <int EB>
+__device__ __forceinline__ void chunk_statistics(const uint32_t* w, int jq, int jlim, uint8_t* dump_row, uint32_t* uf,
+                                                 int n_sink) {
+    constexpr int NW = 8 * EB;      // words of the chunk
+    if (dump_row == nullptr && uf == nullptr) return;
+    if (dump_row == nullptr && jq >= n_sink && jq + 31 <= jlim) {
+        // every key of the chunk is visible and none is a sink: count the zero codes a word at a time
+        uint32_t zeros = 0;
+#pragma unroll
+        for (int i = 0; i < NW; ++i)
+            zeros += (EB == 1) ? (__popc(__vcmpeq4(w[i], 0u)) >> 3) : (__popc(__vcmpeq2(w[i], 0u)) >> 4);
+        *uf += zeros;
+        return;
+    }
+    uint32_t zeros = 0;
+#pragma unroll
+    for (int e = 0; e < 32; ++e) {
+        uint32_t code;
+        if constexpr (EB == 1) {
+            code = (w[e >> 2] >> (8 * (e & 3))) & 0xFFu;
+        } else {
+            uint32_t back;
+            asm("mul.rn.bf16x2 %0, %1, %2;" : "=r"(back) : "r"(w[e >> 1]), "r"(0x03800380u));   // 2^-120
+            code = (back >> (16 * (e & 1) + 4)) & 0xFFu;
+        }
+        const bool vis = jq + e <= jlim;
+        if (vis && dump_row != nullptr) dump_row[jq + e] = (uint8_t)code;
+        if (vis && jq + e >= n_sink && code == 0) ++zeros;
+    }
+    if (uf != nullptr) *uf += zeros;
+}
+
+// One P quarter: exp / sum / cast (exp_chunk), P over the head of its S quarter, hand-off to the issuer.
+template <int EB, bool FOLD, int NPOLY = 0, bool AUX = false>
+__device__ __forceinline__ void p_quarter(const uint32_t* v, bool mask, uint32_t tS, int quarter, int j0, int jlim,
+                                          uint64_t cl2_2, uint64_t negm_2, uint64_t s_2, uint64_t& sum_a,
+                                          uint64_t& sum_b, uint64_t* bar, int lane, uint8_t* dump_row = nullptr,
+                                          uint32_t* uf = nullptr, int n_sink = 0) {
+    using C = PrefillCfg<EB>;
+    uint32_t w[C::P_COLS / 4];
+    if (mask) exp_chunk<EB, FOLD, true>(v, w, j0 + quarter * 32, jlim, cl2_2, negm_2, s_2, sum_a, sum_b);
+    else exp_chunk<EB, FOLD, false, NPOLY>(v, w, j0 + quarter * 32, jlim, cl2_2, negm_2, s_2, sum_a, sum_b);
+    if constexpr (AUX) chunk_statistics<EB>(w, j0 + quarter * 32, jlim, dump_row, uf, n_sink);
+    if constexpr (EB == 1) ptx::tmem_st_x8(tS + quarter * 32, w);
+    else ptx::tmem_st_x16(tS + quarter * 32, w);
+    ptx::tmem_wait_st();
+    ptx::tc_fence_before();
+    __syncwarp();
+    if (lane == 0) ptx::mbar_arrive(bar);
+}
+
+}  // namespace fp8attn

@@ -56,11 +56,11 @@ __device__ __forceinline__ float load_as_f32<__nv_bfloat16>(const __nv_bfloat16*
 // amax_bits[slab] = bit pattern of max |x| over the slab (non-negative floats order like uints)
 template <typename T>
 __global__ void absmax_kernel(const T* __restrict__ x, unsigned int* __restrict__ amax_bits, long long slab_elems) {
-    const long long slab = blockIdx.y;
+    const long long slab = blockIdx.x;            // grid = (slabs, chunks of the slab)
     const T* xs = x + slab * slab_elems;
     float m = 0.0f;
-    for (long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x; i < slab_elems;
-         i += (long long)gridDim.x * blockDim.x)
+    for (long long i = (long long)blockIdx.y * blockDim.x + threadIdx.x; i < slab_elems;
+         i += (long long)gridDim.y * blockDim.x)
         m = fmaxf(m, fabsf(load_as_f32<T>(xs, i)));
     for (int o = 16; o > 0; o >>= 1) m = fmaxf(m, __shfl_xor_sync(0xFFFFFFFFu, m, o));
     if ((threadIdx.x & 31) == 0) atomicMax(amax_bits + slab, __float_as_uint(m));
@@ -70,13 +70,13 @@ __global__ void absmax_kernel(const T* __restrict__ x, unsigned int* __restrict_
 template <typename T>
 __global__ void quantize_kernel(const T* __restrict__ x, const unsigned int* __restrict__ amax_bits,
                                 uint8_t* __restrict__ codes, long long slab_elems) {
-    const long long slab = blockIdx.y;
+    const long long slab = blockIdx.x;
     const float amax = __uint_as_float(amax_bits[slab]);
     const float inv = amax > 0.0f ? __fdiv_rn(448.0f, amax) : 1.0f;
     const T* xs = x + slab * slab_elems;
     uint8_t* cs = codes + slab * slab_elems;
-    for (long long i = ((long long)blockIdx.x * blockDim.x + threadIdx.x) * 2; i < slab_elems;
-         i += (long long)gridDim.x * blockDim.x * 2) {
+    for (long long i = ((long long)blockIdx.y * blockDim.x + threadIdx.x) * 2; i < slab_elems;
+         i += (long long)gridDim.y * blockDim.x * 2) {
         const float a = __fmul_rn(load_as_f32<T>(xs, i), inv);
         const float b = (i + 1 < slab_elems) ? __fmul_rn(load_as_f32<T>(xs, i + 1), inv) : 0.0f;
         const uint32_t pr = ptx::cvt_e4m3x2(a, b);

@@ -8,6 +8,7 @@ the tensor-level wrappers `fwd`, `quantize_e4m3` and `debug_gemm`.
 """
 import ctypes as C
 import os
+import subprocess
 from dataclasses import dataclass
 from typing import Optional
 
@@ -37,9 +38,14 @@ class Stats(C.Structure):
 
 
 def _load():
-    path = LIB
-    if not os.path.exists(path):
-        path = build()          # needs nvcc; raises if it cannot build
+    # build() compares modification times and rebuilds a stale library (needs nvcc); without nvcc an
+    # existing library is used as it is
+    try:
+        path = build()
+    except (OSError, subprocess.CalledProcessError):
+        if not os.path.exists(LIB):
+            raise
+        path = LIB
     lib = C.CDLL(path)
     lib.fp8attn_fwd.argtypes = [C.c_void_p] * 4 + [C.c_int] * 7 + [C.c_float, C.c_int, C.c_int,
                                                                   C.POINTER(Stats)]
@@ -54,6 +60,7 @@ def _load():
     lib.fp8attn_strerror.restype = C.c_char_p
     lib.fp8attn_last_cuda_error.restype = C.c_char_p
     lib.fp8attn_version.restype = C.c_int
+    lib.fp8attn_trim.restype = C.c_int
     return lib
 
 
@@ -65,6 +72,7 @@ fp8attn_fwd_host = _lib.fp8attn_fwd_host
 fp8attn_quantize_e4m3 = _lib.fp8attn_quantize_e4m3
 fp8attn_debug_gemm = _lib.fp8attn_debug_gemm
 fp8attn_version = _lib.fp8attn_version
+fp8attn_trim = _lib.fp8attn_trim
 
 
 def fp8attn_strerror(code: int) -> str:
@@ -127,7 +135,7 @@ def fwd(q, k, v, *, causal: bool, S: float, kv_order: int, mode: int, n_sink: in
     """fp8attn_fwd on CUDA tensors q [B,Hq,Lq,d], k/v [B,Hkv,Lk,d] (contiguous).  `mode` is the
     P mode (0 no-cast, 1 isolation, 2 FP8); the input dtype bits are derived from the tensors.
     `dump_head=(b,h)` returns the E4M3 code of every P of that head.  `kernel` requests a kernel
-    family (0 automatic; the P dump and the underflow counters exist in the general kernel only)."""
+    family (0 automatic, 1 general, 2 prefill, 3 decode)."""
     for t in (q, k, v):
         if not (t.is_cuda and t.is_contiguous() and t.dim() == 4):
             raise ValueError("q, k, v must be contiguous 4-D CUDA tensors")

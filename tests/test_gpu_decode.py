@@ -1,5 +1,7 @@
 """GPU parity of the split-KV decode kernel (kernel family 3, csrc/attn_decode.cuh) against the CPU
-oracle run with the same split boundaries (reading R14), and against the general kernel."""
+oracle run with the same split boundaries (reading R14): outputs, row statistics, and --
+through the statistics instance of the kernel (same schedule) -- the E4M3 code of every P element by
+element and both underflow counters; and against the general kernel."""
 import numpy as np
 import pytest
 import torch
@@ -36,6 +38,28 @@ def test_decode_kernel_matches_oracle(shape, kind, ns, order, S):
         assert r.num_splits == min(ns, nb)
     ref = P.run_oracle(case, r, causal=causal, S=S, order=order, mode=2)
     P.check(case, r, ref, mode=2, label=f"decode {shape} {kind} ns={ns} S={S} order={order}", check_mse=False)
+    # the statistics instance of the same kernel: every P code of one head against the oracle's (north_star:
+    # >= 99.9 % identical in FP8 mode, never more than one code step apart; Alg. 1 line 9)
+    # and both underflow counters over the whole call (Prop. 1)
+    b, h = B - 1, Hq - 1
+    ra = P.run_gpu(case, causal=causal, S=S, order=order, mode=2, num_splits=r.num_splits, kernel=3, underflow=True,
+                   dump_head=(b, h))
+    assert ra.kernel_id == 3 and ra.split_bounds == r.split_bounds
+    assert torch.equal(ra.o, r.o) and torch.equal(ra.row_max, r.row_max) and torch.equal(ra.row_sum, r.row_sum)
+    rows = (b * Hq + h) * Lq + np.arange(Lq)
+    refc = P.run_oracle(case, ra, causal=causal, S=S, order=order, mode=2, rows=rows, want_codes=True)
+    g = ra.p_codes.cpu().numpy()
+    vis = refc.p_codes != 0xFF
+    assert np.array_equal(g == 0xFF, ~vis), "mask pattern of the P dump differs"
+    n_flip = int(np.sum(g[vis] != refc.p_codes[vis]))
+    assert 1.0 - n_flip / max(1, int(vis.sum())) >= P.CODE_MATCH[2]
+    assert np.abs(g[vis].astype(np.int32) - refc.p_codes[vis].astype(np.int32)).max(initial=0) <= 1
+    uf = ra.underflow.cpu().numpy()
+    slack = max(4, int(2e-3 * ref.n_nonsink_visible))
+    assert abs(int(uf[0]) - ref.uf_sink_block) <= slack, (uf, ref.uf_sink_block)
+    assert abs(int(uf[1]) - ref.uf_other_blocks) <= slack, (uf, ref.uf_other_blocks)
+    if order == 1 and S == 256.0 and r.num_splits == 1:
+        assert int(uf[1]) == 0 == ref.uf_other_blocks          # Thm 4
     # the general kernel with the same split layout
     g = P.run_gpu(case, causal=causal, S=S, order=order, mode=2, num_splits=r.num_splits, kernel=1)
     assert g.kernel_id == 1 and g.split_bounds == r.split_bounds
@@ -51,8 +75,10 @@ def test_decode_is_the_default_for_decode_shapes():
     r = P.run_gpu(case, causal=False, S=256.0, order=1, mode=2, stats=False)
     assert r.kernel_id == 3
     assert r.n_launches == 1 + 1 + (1 if r.num_splits > 1 else 0)     # q quantiser (one fused launch), decode, combine
-    r = P.run_gpu(case, causal=False, S=256.0, order=1, mode=2, stats=True)          # underflow counters wanted
-    assert r.kernel_id == 1
+    r1 = P.run_gpu(case, causal=False, S=256.0, order=1, mode=2, stats=True)         # underflow counters wanted:
+    assert r1.kernel_id == 3 and r1.num_splits == r.num_splits                        # the statistics instance
+    g = P.run_gpu(case, causal=False, S=256.0, order=1, mode=2, stats=True, kernel=1, num_splits=r.num_splits)
+    assert g.kernel_id == 1 and torch.equal(g.underflow, r1.underflow)
     f = P.fa()
     q2, k2, v2 = W.sink_qkv(1, 32, 1, 1, 256, 128, 10.0, seed=1)                     # 32 rows per kv head
     with pytest.raises(f.Fp8AttnError) as e:
