@@ -1,23 +1,18 @@
-// attn_prefill.cuh -- warp-specialised prefill kernel: every softmax warp works on BOTH query tiles.
+// attn_prefill.cuh -- warp-specialised prefill kernel, d = 128, Bn = 128, two 128-row query tiles per CTA.
 //
-// Same arithmetic as attn_general.cuh (Alg. 1: exact running max after every block, l from
-// the FP32 pre-cast P, cvt.rn.satfinite.e4m3x2.f32 of P*S, epilogue O / (S l)); d = 128, Bn = 128, two
-// 128-row query tiles per CTA.  Measured on B200: a successful mbarrier wait costs ~130 cycles, so the chain
-// "last P quarter -> issuer notices -> P.V + QK^T -> commit -> softmax warp notices -> load S" is 600-900
-// cycles during which the softmax warp of that tile has nothing to do.  Here the two softmax warps of a
-// scheduler do not own one tile each; they own one HALF of the key columns of both tiles:
-//   warp (wq, half): rows 32 wq .. 32 wq + 31 of tile 0 and of tile 1, key columns 64 half .. 64 half + 63
-// and alternate between the tiles: while a warp is in the exp pass of tile 1, the tensor pipe turns tile 0
-// around, and vice versa, so the chain is hidden and both warps of a scheduler are in an exp pass together
-// (two warps keep the MUFU pipe ~90 % busy, one alone cannot).  The price is one exchange per block: the two
-// warps of a row pair swap their 64-column maxima through shared memory and a 64-thread named barrier.
-// Each warp loads its 64 logits of a row once, keeps them in registers through max and exp, and sums its
-// own columns (both warps use the same running max, so the partial row sums just add in the epilogue).
-// O <- alpha O (Alg. 1 line 10, first half) is done by a correction warpgroup per tile.
-// Roles (640 threads, register budgets moved with setmaxnreg):
-//   warps 0-3 / 4-7    softmax, column half 0 / 1 (one query row per lane = TMEM lane, both tiles)
-//   warps 8-11 / 12-15 correction of tile 0 / 1
+// Arithmetic as in attn_general.cuh (Alg. 1: exact running max after every block, l from the
+// FP32 pre-cast P, cvt.rn.satfinite.e4m3x2.f32 of P*S, epilogue O / (S l)).  Who does what:
+//   warps 0-3 / 4-7    "exp" warps, key-column half 0 / 1: lane = query row (TMEM lane) of BOTH tiles; Alg. 1
+//                      lines 7-9 (P = exp, row sum from the pre-cast P, cast, P -> TMEM) and line 12
+//   warps 8-11 / 12-15 "max" warps of tile 0 / 1: lines 4-6 (block max over all 128 columns, running max, alpha),
+//                      published to the exp warps through shared memory, then O <- alpha O in TMEM (line 10)
 //   warps 16, 17       tcgen05.mma issuers of tile 0 / 1;  warp 18 TMA producer;  19 idle
+// Why: the exp pass is the MUFU-bound part of the kernel (16 ex2 / clk / SM against 16384 FP8 FLOP / clk), so the
+// warps that run it do nothing else.  An exp warp alternates between the two tiles -- (it, tile 1), (it, tile 0),
+// (it + 1, tile 1) ... -- and while it is in the exp pass of one tile, the tensor pipe turns the other tile
+// around (P.V, QK^T of the next block) and the max warp of that tile reduces the new S.  The row maximum needs
+// all 128 columns of a row, the exp pass splits them between two warps: with the maximum computed by a third
+// warp there is no exchange between the two (round 1 swapped 64-column maxima through a named barrier).
 // TMEM (512 columns): S0 [0,128) S1 [128,256) O0 [256,384) O1 [384,512); P over the head of each S quarter.
 #pragma once
 #include "prefill_common.cuh"
@@ -32,24 +27,88 @@ struct PrefillKCfg {
     // which of the 16 element pairs of a P quarter take the FMA-pipe exp2.  BF16 operands: none (measured: the
     // BF16 mode has twice the tensor time and the extra code-to-BF16 conversion, the polynomial costs 6 % there)
     static constexpr int NPOLY = (EB == 1) ? 0x8080 : 0;
-    // q_full[2] k_full/k_empty/v_full/v_empty[NS] s_full[2] p_full[2][2] a_full[2][4] o_ready[2] o_done[2]
+    // q_full[2] k_full/k_empty/v_full/v_empty[NS] s_full[2] p_full[2][2] m_full[2][4] o_ready[2] o_done[2]
     static constexpr int N_BARS = 2 + 4 * P::NS + 2 + 4 + 8 + 2 + 2;
-    // + alpha[2][128] + mx[2 tiles][2 block parities][2 halves][128 rows]
-    static constexpr int SMEM_BYTES = (2 + 2 * P::NS) * P::TILE + 1024 /*align*/ + N_BARS * 8 + 16 + 2 * 128 * 4 +
-                                      2 * 2 * 2 * 128 * 4;
-    static constexpr int REG_SOFTMAX = 144, REG_CORR = 72, REG_MISC = 40;   // 256 (144 + 72) + 128 * 40 <= 640 * 96
+    // + mstat[2 tiles][2 block parities][128 rows] float2 + lsum[2 tiles][2 halves][128 rows] float
+    static constexpr int SMEM_BYTES = (2 + 2 * P::NS) * P::TILE + 1024 /*align*/ + N_BARS * 8 + 16 + 2 * 2 * 128 * 8 +
+                                      2 * 2 * 128 * 4;
+    static constexpr int REG_EXP = 128, REG_MAX = 80, REG_MISC = 56;   // 256 (128 + 80) + 128 * 56 <= 640 * 96
 };
 
-// ---- correction warp: O <- alpha O for its 32 rows, once per block ---------------------------------
-__device__ __forceinline__ void prefill_correction(int t, int wq, int lane, uint32_t tbase, uint64_t* a_full_w,
-                                                    const float* alpha_slot, uint64_t* o_ready, int n_t) {
-    const uint32_t tO = tbase + (static_cast<uint32_t>(wq * 32) << 16) + 256 + t * 128;
+// Which blocks of a tile need the mask for some row of the 32-row group `wq`: blocks whose first key index
+// exceeds the returned value (bottom-right causal diagonal, tail of the sequence; reading R15).
+__device__ __forceinline__ int mask_threshold(const FwdParams& p, int row0, int wq) {
+    const long long wvis = p.causal ? (long long)row0 + wq * 32 + (p.Lk - p.Lq) : (long long)p.Lk - 1;
+    long long thr = wvis - 127 < (long long)p.Lk - 128 ? wvis - 127 : (long long)p.Lk - 128;
+    if (thr < -(1ll << 30)) thr = -(1ll << 30);
+    return (int)thr;
+}
+__device__ __forceinline__ int last_visible_key(const FwdParams& p, int qrow) {
+    long long jl = p.causal ? (long long)qrow + (p.Lk - p.Lq) : (long long)p.Lk - 1;
+    if (jl > p.Lk - 1) jl = p.Lk - 1;
+    return (int)jl;       // negative: the row sees no key
+}
+
+// What a max warp publishes per (tile, block, row) for the exp warps: the exponent offset of line 7,
+// -m_new c log2(e) (+ log2 S when the scale is folded), and alpha of line 6.
+struct RowStat {
+    float negm, alpha;
+};
+
+// ---- max warp (t, wq): Alg. 1 lines 4-6 for rows 32 wq .. 32 wq + 31 of tile t, then O <- alpha O ----
+template <int EB, bool FOLD>
+__device__ __forceinline__ void prefill_max_warp(const FwdParams& p, int t, int wq, int lane, uint32_t tbase,
+                                                 uint64_t* s_full_t, uint64_t* m_full_w, RowStat* mstat_t,
+                                                 uint64_t* o_ready_t, int n_t, int row0, int bh, int kvh) {
+    using C = PrefillCfg<EB>;
+    const uint32_t tlane = tbase + (static_cast<uint32_t>(wq * 32) << 16);
+    const uint32_t tS = tlane + C::TM_S + t * 128, tO = tlane + C::TM_O + t * 128;
+    const int rl = wq * 32 + lane;
+    const int jlim = last_visible_key(p, row0 + rl);
+    const int mask_from = mask_threshold(p, row0, wq);
+    float c_nat = p.sm_scale;
+    if constexpr (EB == 1) c_nat *= p.q_scale[bh] * p.k_scale[kvh];
+    const float cl2 = c_nat * LOG2E;
+    const float log2S = FOLD ? log2f(p.S) : 0.0f;   // exact for S = 2^k
+    float m_run = -INFINITY;
+
+#pragma unroll 1
     for (int c = 0; c < n_t; ++c) {
-        ptx::mbar_wait(a_full_w, c & 1);
-        const float alpha = *alpha_slot;
-        // alpha(c) is published after S(c) is complete, which implies P.V(c-1) is complete (in-order pipe)
+        const int blk = (p.kv_order == 0) ? c : n_t - 1 - c;
+        const int j0 = blk * 128;
+        const bool mask = j0 > mask_from;
+        ptx::mbar_wait(s_full_t, c & 1);
+        ptx::tc_fence_after();
+        // ---- line 4: block max over the 128 columns of the row.  A TMEM load takes ~300 cycles to come back while
+        // the tensor pipe is busy and tcgen05.wait::ld waits for every load in flight: two round trips of 64 columns ----
+        float m0 = -INFINITY, m1 = -INFINITY;
+#pragma unroll
+        for (int hb = 0; hb < 2; ++hb) {
+            uint32_t v[64];
+            ptx::tmem_ld_x32(tS + hb * 64, v);
+            ptx::tmem_ld_x32(tS + hb * 64 + 32, v + 32);
+            ptx::tmem_wait_ld();
+            if (mask) {
+                mask32(v, j0 + hb * 64, jlim);
+                mask32(v + 32, j0 + hb * 64 + 32, jlim);
+            }
+#pragma unroll
+            for (int e = 0; e < 64; e += 4) {
+                m0 = fmaxf(fmaxf(m0, __uint_as_float(v[e])), __uint_as_float(v[e + 1]));
+                m1 = fmaxf(fmaxf(m1, __uint_as_float(v[e + 2])), __uint_as_float(v[e + 3]));
+            }
+        }
+        // ---- lines 5-6 ----
+        const float m_new = fmaxf(m_run, fmaxf(m0, m1));
+        const float m_used = (m_new == -INFINITY) ? 0.0f : m_new;
+        const float alpha = ptx::ex2_approx((m_run - m_used) * cl2);       // 0 when m_run = -inf
+        const float negm = fmaf(-m_used, cl2, log2S);
+        m_run = m_new;
+        ptx::st_shared_v2(mstat_t + (c & 1) * 128 + rl, negm, alpha);
+        __syncwarp();
+        if (lane == 0) ptx::mbar_arrive(m_full_w);
+        // ---- line 10, first half: O <- alpha O.  S(c) complete implies P.V(c-1) complete (in-order pipe) ----
         if (c > 0 && __any_sync(0xFFFFFFFFu, alpha != 1.0f)) {
-            ptx::tc_fence_after();
             const uint64_t a2 = ptx::pack2(alpha, alpha);
             uint32_t va[16], vb[16];
             ptx::tmem_ld_x16(tO, va);
@@ -72,23 +131,42 @@ __device__ __forceinline__ void prefill_correction(int t, int wq, int lane, uint
         }
         ptx::tc_fence_before();
         __syncwarp();
-        if (lane == 0) ptx::mbar_arrive(o_ready);
+        if (lane == 0) ptx::mbar_arrive(o_ready_t);
     }
+    // statistics: the final running max (natural-log units of the scaled logit)
+    const int qrow = row0 + rl;
+    if (p.row_max != nullptr && qrow < p.Lq)
+        p.row_max[(long long)bh * p.Lq + qrow] = (m_run == -INFINITY) ? -INFINITY : m_run * c_nat;
 }
 
-// ---- softmax warp (wq, half): Alg. 1 lines 4-9 and 12 for its rows of both tiles, its 64 key columns ----
-template <int EB, bool FOLD, bool AUX>
-__device__ __forceinline__ void prefill_softmax(const FwdParams& p, int wq, int half, int lane, uint32_t tbase,
-                                                 uint64_t* s_full, uint64_t* p_full, uint64_t* a_full, float* alpha_s,
-                                                 float* mx, uint64_t* o_done, const int* n_tile, int n_it, int pair,
-                                                 int bh, int kvh, const CUtensorMap* mapO, uint8_t* stage0,
-                                                 uint8_t* stage1) {
+// One P quarter: exp / sum / cast (exp_chunk), statistics (AUX), P over the head of its S quarter in TMEM (the A
+// operand of P.V), arrival on the issuer's barrier.
+template <int EB, bool FOLD, int NPOLY, bool AUX>
+__device__ __forceinline__ void p_quarter(const uint32_t* v, uint32_t tS, int quarter, int j0, int jlim, uint64_t cl2_2,
+                                          uint64_t negm_2, uint64_t s_2, uint64_t& sum_a, uint64_t& sum_b, uint64_t* bar,
+                                          int lane, uint8_t* dump_row, uint32_t* uf, int n_sink) {
     using C = PrefillCfg<EB>;
-    using C4 = PrefillKCfg<EB>;
+    uint32_t w[C::P_COLS / 4];
+    exp_chunk<EB, FOLD, false, NPOLY>(v, w, j0 + quarter * 32, jlim, cl2_2, negm_2, s_2, sum_a, sum_b);
+    if constexpr (AUX) chunk_statistics<EB>(w, j0 + quarter * 32, jlim, dump_row, uf, n_sink);
+    if constexpr (EB == 1) ptx::tmem_st_x8(tS + quarter * 32, w);
+    else ptx::tmem_st_x16(tS + quarter * 32, w);
+    ptx::tmem_wait_st();
+    ptx::tc_fence_before();
+    __syncwarp();
+    if (lane == 0) ptx::mbar_arrive(bar);
+}
+
+// ---- exp warp (wq, half): Alg. 1 lines 7-9 and 12 for its rows of both tiles, its 64 key columns ----
+template <int EB, bool FOLD, bool AUX>
+__device__ __forceinline__ void prefill_exp_warp(const FwdParams& p, int wq, int half, int lane, uint32_t tbase,
+                                                 uint64_t* m_full, uint64_t* p_full, const RowStat* mstat, float* lsum,
+                                                 uint64_t* o_done, const int* n_tile, int n_it, int pair, int bh,
+                                                 int kvh, const CUtensorMap* mapO, uint8_t* stage0, uint8_t* stage1) {
+    using C = PrefillCfg<EB>;
+    using CK = PrefillKCfg<EB>;
     const uint32_t tlane = tbase + (static_cast<uint32_t>(wq * 32) << 16);
     const int rl = wq * 32 + lane;              // row within the tile = TMEM lane
-    const int off = p.Lk - p.Lq;
-    const int bar_id = 1 + wq;                  // named barrier of the two warps that share these rows
 
     float c_nat = p.sm_scale, vs = 1.0f;
     if constexpr (EB == 1) {
@@ -96,34 +174,26 @@ __device__ __forceinline__ void prefill_softmax(const FwdParams& p, int wq, int 
         vs = p.v_scale[kvh];
     }
     const float cl2 = c_nat * LOG2E;
-    const float log2S = FOLD ? log2f(p.S) : 0.0f;   // exact for S = 2^k
     const uint64_t cl2_2 = ptx::pack2(cl2, cl2), s_2 = ptx::pack2(p.S, p.S);
 
-    int jlim[2], first[2];
+    int jlim[2], first[2], mask_from[2];
     uint8_t* dump_row[2];     // AUX: this row of the P dump (fp8attn_stats.p_codes), else null
     uint32_t uf_sink = 0, uf_other = 0;   // AUX: zero codes among visible non-sink keys (sink block / other blocks)
-    int mask_from[2];         // blocks whose first key index exceeds this need the mask for some row of the warp
-    float m_run[2] = {-INFINITY, -INFINITY}, l_run[2] = {0.0f, 0.0f};
+    float l_run[2] = {0.0f, 0.0f};
 #pragma unroll
     for (int t = 0; t < 2; ++t) {
         const int row0 = (pair * 2 + t) * BM;
-        long long jl = p.causal ? (long long)row0 + rl + off : (long long)p.Lk - 1;
-        if (jl > p.Lk - 1) jl = p.Lk - 1;
-        jlim[t] = (int)jl;
-        // a block j0 .. j0 + 127 is unmasked iff every row of the warp sees all of it and it lies inside Lk
-        const long long wvis = p.causal ? (long long)row0 + wq * 32 + off : (long long)p.Lk - 1;
-        long long thr = wvis - 127 < (long long)p.Lk - 128 ? wvis - 127 : (long long)p.Lk - 128;
-        if (thr < -(1ll << 30)) thr = -(1ll << 30);
-        mask_from[t] = (int)thr;
+        jlim[t] = last_visible_key(p, row0 + rl);
+        mask_from[t] = mask_threshold(p, row0, wq);
         first[t] = (p.kv_order == 0) ? 0 : n_it - n_tile[t];
         dump_row[t] = (AUX && p.p_codes != nullptr && bh == p.p_bh && row0 + rl < p.Lq)
                           ? p.p_codes + (size_t)(row0 + rl) * p.Lk
                           : nullptr;
     }
 
-    // A successful mbarrier wait takes ~130 cycles to report.  When the next block belongs to the other tile its
-    // S has been ready for a while, so the barrier is probed before the second P quarter of the current block
-    // and the answer is read when the next block starts (probed_tile >= 0: a probe is pending).
+    // A successful mbarrier wait takes ~100 cycles to report.  When the next block belongs to the other tile its
+    // running max has been ready for a while, so that barrier is probed before the second P quarter of the
+    // current block and the answer is read when the next block starts (probed_tile >= 0: a probe is pending).
     FP8ATTN_DECL_PROBE_PRED();
     int probed_tile = -1;
 #pragma unroll 1
@@ -141,33 +211,20 @@ __device__ __forceinline__ void prefill_softmax(const FwdParams& p, int wq, int 
             const int j0 = blk * 128;
             const bool mask = j0 > mask_from[t];
             const uint32_t tS = tlane + C::TM_S + t * 128;
-            // ---- this warp's 64 logits of the row, loaded once ----
+            // ---- the running max of block c is published (which implies S(c) is complete): this warp's 64
+            // logits of the row, loaded once ----
             uint32_t r[64];
-            if (probed_tile != t || !ptx::mbar_probe_result()) ptx::mbar_wait(s_full + t, c & 1);
+            if (probed_tile != t || !ptx::mbar_probe_result()) ptx::mbar_wait(m_full + 4 * t + wq, c & 1);
             probed_tile = -1;
             ptx::tc_fence_after();
             ptx::tmem_ld_x32(tS + half * 64, r);
             ptx::tmem_ld_x32(tS + half * 64 + 32, r + 32);
+            const float2 ms = ptx::ld_shared_v2(mstat + (t * 2 + (c & 1)) * 128 + rl);   // (negm, alpha)
+            const uint64_t negm_2 = ptx::pack2(ms.x, ms.x);
             ptx::tmem_wait_ld();
             if (mask) {
                 mask32(r, j0 + half * 64, jlim[t]);
                 mask32(r + 32, j0 + half * 64 + 32, jlim[t]);
-            }
-            // ---- lines 4-6: block max (exchanged with the warp of the other column half), running max ----
-            float mloc = fmaxf(max32(r, -INFINITY), max32(r + 32, -INFINITY));
-            float* mxt = mx + (t * 2 + (c & 1)) * 256;
-            mxt[half * 128 + rl] = mloc;
-            ptx::named_bar_sync(bar_id, 64);
-            mloc = fmaxf(mloc, mxt[(half ^ 1) * 128 + rl]);
-            const float m_new = fmaxf(m_run[t], mloc);
-            const float m_used = (m_new == -INFINITY) ? 0.0f : m_new;
-            const float alpha = ptx::ex2_approx((m_run[t] - m_used) * cl2);   // 0 when m_run = -inf
-            const float negm = fmaf(-m_used, cl2, log2S);
-            const uint64_t negm_2 = ptx::pack2(negm, negm);
-            if (half == 0) {                    // alpha goes to the correction warp of these rows
-                alpha_s[t * 128 + rl] = alpha;
-                __syncwarp();
-                if (lane == 0) ptx::mbar_arrive(a_full + 4 * t + wq);
             }
             // ---- lines 7-9: two P quarters ----
             uint64_t sum_a = ptx::pack2(0.f, 0.f), sum_b = sum_a;
@@ -179,19 +236,18 @@ __device__ __forceinline__ void prefill_softmax(const FwdParams& p, int wq, int 
             uint32_t* const uf = (AUX && p.underflow != nullptr && (pair * 2 + t) * BM + rl < p.Lq)
                                      ? (j0 < p.n_sink ? &uf_sink : &uf_other)
                                      : nullptr;
-            p_quarter<EB, FOLD, C4::NPOLY, AUX>(r, false, tS, 2 * half, j0, jlim[t], cl2_2, negm_2, s_2, sum_a, sum_b,
+            p_quarter<EB, FOLD, CK::NPOLY, AUX>(r, tS, 2 * half, j0, jlim[t], cl2_2, negm_2, s_2, sum_a, sum_b,
                                                 p_full + 2 * t + 0, lane, dump_row[t], uf, p.n_sink);
             if (probe_next) {
-                ptx::mbar_probe(s_full + (t ^ 1), c_o & 1);
+                ptx::mbar_probe(m_full + 4 * (t ^ 1) + wq, c_o & 1);
                 probed_tile = t ^ 1;
             }
-            p_quarter<EB, FOLD, C4::NPOLY, AUX>(r + 32, false, tS, 2 * half + 1, j0, jlim[t], cl2_2, negm_2, s_2, sum_a,
+            p_quarter<EB, FOLD, CK::NPOLY, AUX>(r + 32, tS, 2 * half + 1, j0, jlim[t], cl2_2, negm_2, s_2, sum_a,
                                                 sum_b, p_full + 2 * t + 1, lane, dump_row[t], uf, p.n_sink);
             float sa, sb, sc, sd;
             ptx::unpack2(sum_a, sa, sb);
             ptx::unpack2(sum_b, sc, sd);
-            l_run[t] = alpha * l_run[t] + ((sa + sb) + (sc + sd));   // line 8 (this warp's columns)
-            m_run[t] = m_new;
+            l_run[t] = ms.y * l_run[t] + ((sa + sb) + (sc + sd));   // line 8 (this warp's columns)
         }
     }
 
@@ -204,9 +260,14 @@ __device__ __forceinline__ void prefill_softmax(const FwdParams& p, int wq, int 
             }
         }
     }
-    // ---- line 12: O / (S l), statistics.  Each warp owns 32 rows x 64 output columns of each tile: it scales
-    // them, writes them as two 32-row x 128-byte boxes (128-byte swizzle) into the K / V ring, which no MMA reads
-    // any more once both tiles are done, and stores the boxes with TMA (rows >= Lq are clipped by the map) ----
+    // ---- line 12: O / (S l), row sum.  The two warps of a row add their partial sums (same running max, so they
+    // just add).  Each warp owns 32 rows x 64 output columns of each tile: it scales them, writes them as two
+    // 32-row x 128-byte boxes (128-byte swizzle) into the K / V ring, which no MMA reads any more once both tiles
+    // are done, and stores the boxes with TMA (rows >= Lq are clipped by the map) ----
+#pragma unroll
+    for (int t = 0; t < 2; ++t)
+        lsum[(t * 2 + half) * 128 + rl] = (jlim[t] < 0) ? 0.0f : l_run[t];     // no visible key: l = 0 exactly
+    ptx::named_bar_sync(1 + wq, 64);            // the two warps that share these rows
 #pragma unroll
     for (int t = 0; t < 2; ++t) {
         if (n_tile[t] > 0) ptx::mbar_wait(o_done + t, 0);
@@ -216,18 +277,9 @@ __device__ __forceinline__ void prefill_softmax(const FwdParams& p, int wq, int 
     for (int t = 0; t < 2; ++t) {
         const int row0 = (pair * 2 + t) * BM;
         const int qrow = row0 + rl;
-        const long long grow = (long long)bh * p.Lq + qrow;
-        float* mxt = mx + t * 512;
-        ptx::named_bar_sync(bar_id, 64);        // the partner has read the last block maximum
-        const float l_mine = (m_run[t] == -INFINITY) ? 0.0f : l_run[t];   // no visible key: l = 0 exactly
-        mxt[half * 128 + rl] = l_mine;
-        ptx::named_bar_sync(bar_id, 64);
-        const float l_all = l_mine + mxt[(half ^ 1) * 128 + rl];
-        const float l_true = FOLD ? l_all / p.S : l_all;
-        if (qrow < p.Lq && half == 0) {
-            if (p.row_max) p.row_max[grow] = (m_run[t] == -INFINITY) ? -INFINITY : m_run[t] * c_nat;
-            if (p.row_sum) p.row_sum[grow] = l_true;
-        }
+        const float l_all = lsum[(t * 2) * 128 + rl] + lsum[(t * 2 + 1) * 128 + rl];
+        if (qrow < p.Lq && half == 0 && p.row_sum != nullptr)
+            p.row_sum[(long long)bh * p.Lq + qrow] = FOLD ? l_all / p.S : l_all;
         const float inv = (l_all > 0.0f) ? (FOLD ? vs / l_all : vs / (p.S * l_all)) : 0.0f;
         if (row0 >= p.Lq) continue;             // no row of this tile exists (warp-uniform)
         const uint32_t tO = tlane + C::TM_O + t * 128 + half * 64;
@@ -260,7 +312,6 @@ __device__ __forceinline__ void prefill_softmax(const FwdParams& p, int wq, int 
         ptx::bulk_wait_group_read0();
     }
 }
-
 // ---- the kernel ---------------------------------------------------------------------------------
 // grid = ceil(Lq / 256) * B*Hq CTAs in one dimension (order: see below).
 template <int EB, bool FOLD, bool AUX = false>
@@ -281,14 +332,14 @@ attn_prefill_kernel(const __grid_constant__ CUtensorMap mapQ, const __grid_const
     uint64_t* k_empty = k_full + C::NS;
     uint64_t* v_full = k_empty + C::NS;
     uint64_t* v_empty = v_full + C::NS;
-    uint64_t* s_full = v_empty + C::NS;           // [2 tiles]                   MMA -> softmax
-    uint64_t* p_full = s_full + 2;                // [2 tiles][2 steps]          softmax (8 warps) -> MMA
-    uint64_t* a_full = p_full + 4;                // [2 tiles][4 warps]          softmax warp -> correction warp
-    uint64_t* o_ready = a_full + 8;               // [2]                         correction (4 warps) -> MMA
+    uint64_t* s_full = v_empty + C::NS;           // [2 tiles]                   MMA -> max warps
+    uint64_t* p_full = s_full + 2;                // [2 tiles][2 steps]          exp warps (8) -> MMA
+    uint64_t* m_full = p_full + 4;                // [2 tiles][4 row groups]     max warp -> its two exp warps
+    uint64_t* o_ready = m_full + 8;               // [2]                         max warps (4) -> MMA
     uint64_t* o_done = o_ready + 2;               // [2]
     uint32_t* tmem_slot = reinterpret_cast<uint32_t*>(o_done + 2);
-    float* alpha_s = reinterpret_cast<float*>(tmem_slot + 4);   // [2 tiles][128 rows]
-    float* mx = alpha_s + 256;                                  // [2 tiles][2 parities][2 halves][128 rows]
+    RowStat* mstat = reinterpret_cast<RowStat*>(tmem_slot + 4);   // [2 tiles][2 block parities][128 rows]
+    float* lsum = reinterpret_cast<float*>(mstat + 2 * 2 * 128);  // [2 tiles][2 halves][128 rows]
 
     const int tid = threadIdx.x, lane = tid & 31;
     const int warp = __shfl_sync(0xFFFFFFFFu, tid >> 5, 0);   // provably warp-uniform
@@ -341,7 +392,7 @@ attn_prefill_kernel(const __grid_constant__ CUtensorMap mapQ, const __grid_const
             ptx::mbar_init(o_done + i, 1);
         }
         for (int i = 0; i < 4; ++i) ptx::mbar_init(p_full + i, 8);
-        for (int i = 0; i < 8; ++i) ptx::mbar_init(a_full + i, 1);
+        for (int i = 0; i < 8; ++i) ptx::mbar_init(m_full + i, 1);
         ptx::fence_mbar_init();
     }
     if (warp == 16) {
@@ -354,14 +405,14 @@ attn_prefill_kernel(const __grid_constant__ CUtensorMap mapQ, const __grid_const
     const uint32_t tbase = *tmem_slot;
 
     if (warp < 8) {
-        ptx::setmaxnreg_inc<C4::REG_SOFTMAX>();
-        prefill_softmax<EB, FOLD, AUX>(p, warp & 3, warp >> 2, lane, tbase, s_full, p_full, a_full, alpha_s, mx, o_done,
-                                   n_tile, n_it, pair, bh, kvh, &mapO, sK, sV);
+        ptx::setmaxnreg_inc<C4::REG_EXP>();
+        prefill_exp_warp<EB, FOLD, AUX>(p, warp & 3, warp >> 2, lane, tbase, m_full, p_full, mstat, lsum, o_done, n_tile,
+                                        n_it, pair, bh, kvh, &mapO, sK, sV);
     } else if (warp < 16) {
-        ptx::setmaxnreg_dec<C4::REG_CORR>();
+        ptx::setmaxnreg_dec<C4::REG_MAX>();
         const int t = (warp - 8) >> 2, wq = warp & 3;
-        prefill_correction(t, wq, lane, tbase, a_full + 4 * t + wq, alpha_s + t * 128 + wq * 32 + lane, o_ready + t,
-                            n_tile[t]);
+        prefill_max_warp<EB, FOLD>(p, t, wq, lane, tbase, s_full + t, m_full + 4 * t + wq, mstat + t * 2 * 128,
+                                   o_ready + t, n_tile[t], (pair * 2 + t) * BM, bh, kvh);
     } else {
         ptx::setmaxnreg_dec<C4::REG_MISC>();
         if (warp == 18) {

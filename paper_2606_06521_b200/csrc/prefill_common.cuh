@@ -162,23 +162,4 @@ __device__ __forceinline__ void chunk_statistics(const uint32_t* w, int jq, int 
     if (uf != nullptr) *uf += zeros;
 }
 
-// One P quarter: exp / sum / cast (exp_chunk), P over the head of its S quarter, hand-off to the issuer.
-template <int EB, bool FOLD, int NPOLY = 0, bool AUX = false>
-__device__ __forceinline__ void p_quarter(const uint32_t* v, bool mask, uint32_t tS, int quarter, int j0, int jlim,
-                                          uint64_t cl2_2, uint64_t negm_2, uint64_t s_2, uint64_t& sum_a,
-                                          uint64_t& sum_b, uint64_t* bar, int lane, uint8_t* dump_row = nullptr,
-                                          uint32_t* uf = nullptr, int n_sink = 0) {
-    using C = PrefillCfg<EB>;
-    uint32_t w[C::P_COLS / 4];
-    if (mask) exp_chunk<EB, FOLD, true>(v, w, j0 + quarter * 32, jlim, cl2_2, negm_2, s_2, sum_a, sum_b);
-    else exp_chunk<EB, FOLD, false, NPOLY>(v, w, j0 + quarter * 32, jlim, cl2_2, negm_2, s_2, sum_a, sum_b);
-    if constexpr (AUX) chunk_statistics<EB>(w, j0 + quarter * 32, jlim, dump_row, uf, n_sink);
-    if constexpr (EB == 1) ptx::tmem_st_x8(tS + quarter * 32, w);
-    else ptx::tmem_st_x16(tS + quarter * 32, w);
-    ptx::tmem_wait_st();
-    ptx::tc_fence_before();
-    __syncwarp();
-    if (lane == 0) ptx::mbar_arrive(bar);
-}
-
 }  // namespace fp8attn

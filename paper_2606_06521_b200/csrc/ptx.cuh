@@ -37,6 +37,19 @@ __device__ __forceinline__ bool elect_one() {
     return pred != 0;
 }
 
+// explicit shared-memory accesses (a pointer that went through a function argument is generic to the compiler)
+__device__ __forceinline__ void st_shared_v2(const void* p, float a, float b) {
+    asm volatile("st.shared.v2.f32 [%0], {%1, %2};" ::"r"(smem_u32(p)), "f"(a), "f"(b) : "memory");
+}
+__device__ __forceinline__ void st_shared_v4(const void* p, uint32_t a, uint32_t b, uint32_t c, uint32_t d) {
+    asm volatile("st.shared.v4.b32 [%0], {%1, %2, %3, %4};" ::"r"(smem_u32(p)), "r"(a), "r"(b), "r"(c), "r"(d) : "memory");
+}
+__device__ __forceinline__ float2 ld_shared_v2(const void* p) {
+    float2 r;
+    asm volatile("ld.shared.v2.f32 {%0, %1}, [%2];" : "=f"(r.x), "=f"(r.y) : "r"(smem_u32(p)) : "memory");
+    return r;
+}
+
 // ---------------------------------------------------------------- mbarrier
 __device__ __forceinline__ void mbar_init(uint64_t* bar, uint32_t count) {
     asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(bar)), "r"(count) : "memory");
@@ -92,12 +105,13 @@ __device__ __forceinline__ void mbar_wait(uint64_t* bar, uint32_t parity) {
     }
 }
 
-// Split-phase probe: mbarrier.try_wait takes ~130 cycles to return its predicate (measured on B200).  The probe
+// Split-phase probe: an mbarrier wait takes ~100-150 cycles to return its predicate (measured on B200).  The probe
 // writes a function-scope predicate (declared once per kernel with FP8ATTN_DECL_PROBE_PRED), the warp keeps
-// issuing independent work, and mbar_probe_result() reads the predicate later.
+// issuing independent work, and mbar_probe_result() reads the predicate later.  test_wait, not try_wait: a
+// try_wait on a phase that is not complete yet suspends the warp, a probe must never block.
 #define FP8ATTN_DECL_PROBE_PRED() asm volatile(".reg .pred fp8attn_probe_p;")
 __device__ __forceinline__ void mbar_probe(uint64_t* bar, uint32_t parity) {
-    asm volatile("mbarrier.try_wait.parity.shared::cta.b64 fp8attn_probe_p, [%0], %1;" ::"r"(smem_u32(bar)), "r"(parity)
+    asm volatile("mbarrier.test_wait.parity.shared::cta.b64 fp8attn_probe_p, [%0], %1;" ::"r"(smem_u32(bar)), "r"(parity)
                  : "memory");
 }
 __device__ __forceinline__ bool mbar_probe_result() {
