@@ -1,6 +1,6 @@
 """The paper's experiment grid on the CUDA path.
 
-    python -m paper_2606_06521_b200.experiments --exp table1|exp1|exp2|ttest [--seeds K] [--json]
+    python -m paper_2606_06521_b200.experiments --exp table1|exp1|exp2|ttest|cfg2 [--seeds K]
 
 Every number is computed by `fp8attn_fwd` on a B200: the P-cast runs in isolation mode (FP32 Q, K, V; P cast
 to E4M3 at scale S) and the error is taken against the no-cast mode of the same library
@@ -13,6 +13,9 @@ Set-ups (all synthetic, as in the paper; inputs from `workloads.sink_qkv`):
   exp1    PAPER.md:355-362  Delta in [4,13], N=4096, d=128, q_len=32, B=64, k_sink=4; the five configurations
   exp2    PAPER.md:366, 378-388 (Table 2)  Delta=7, N in {512 .. 16384}
   ttest   PAPER.md:474-485 (App. B)  paired t statistic of MSE(Fwd+256) - MSE(Rev+256) over instances
+  cfg2    BASELINE.json configs[1]  B=1, H=8, L=2048, d=128, Delta = 0 .. 14 in steps of 0.5, S in {1,16,256,448}, both
+          orders: MSE and underflow fraction next to Eq. 7.  (The same sweep held against the CPU
+          oracle point by point is tests/cfg2_sweep.py; its table is profiles/cfg2_sweep.md.)
 The paper's numbers are context (another implementation, hardware not stated), not targets.
 """
 import argparse
@@ -129,9 +132,45 @@ def ttest(instances: int = 100, cases=((7.0, 4096), (7.0, 16384), (10.0, 16384),
     return out
 
 
+def delta_k(k: int = 4) -> float:
+    """E[max of k standard normals] (Eq. 3) by trapezoidal quadrature."""
+    m = np.linspace(-10.0, 10.0, 200001)
+    phi = np.exp(-0.5 * m * m) / math.sqrt(2.0 * math.pi)
+    Phi = 0.5 * (1.0 + np.vectorize(math.erf)(m / math.sqrt(2.0)))
+    return float(np.trapz(m * k * phi * Phi ** (k - 1), m))
+
+
+def eq7(delta: float, S: float, k_sink: int = 4) -> float:
+    """Leading-order underflow fraction F(Delta, S) = Phi(Delta + delta_k - 10 ln 2 - ln S) (Eq. 7)."""
+    x = delta + delta_k(k_sink) - 10.0 * math.log(2.0) - math.log(S)
+    return 0.5 * (1.0 + math.erf(x / math.sqrt(2.0)))
+
+
+def cfg2(deltas=tuple(0.5 * i for i in range(29)), scales=(1.0, 16.0, 256.0, 448.0)):
+    cfg = W.CONFIGS["cfg2"]
+    q, k, v = W.config_qkv(cfg, seed=0, delta=0.0)
+    tq, tk, tv = _dev(q), _dev(k), _dev(v)
+    dk = delta_k(cfg.n_sink)
+    out = []
+    for d in deltas:
+        tk[..., :cfg.n_sink, cfg.d - 1] = float(np.float32(d * math.sqrt(cfg.d)))
+        ref = fa.fwd(tq, tk, tv, causal=False, S=1.0, kv_order=0, mode=0, block_n=BLOCK).o.double()
+        for S in scales:
+            for order in (0, 1):
+                r = fa.fwd(tq, tk, tv, causal=False, S=S, kv_order=order, mode=1, block_n=BLOCK, want_stats=True)
+                uf = r.underflow.cpu().numpy().astype(np.float64)
+                frac = float(uf.sum() / (cfg.B * cfg.Hq * cfg.Lq * (cfg.Lk - cfg.n_sink)))
+                x = d + dk - 10.0 * math.log(2.0) - math.log(S)
+                out.append({"exp": "cfg2", "delta": d, "S": S, "order": "rev" if order else "fwd",
+                            "mse": float(((r.o.double() - ref) ** 2).mean().item()),
+                            "underflow_sink_block": int(uf[0]), "underflow_other_blocks": int(uf[1]),
+                            "underflow_fraction": frac, "eq7": 0.5 * (1.0 + math.erf(x / math.sqrt(2.0)))})
+    return out
+
+
 def main(argv=None):
     ap = argparse.ArgumentParser(description=__doc__, formatter_class=argparse.RawDescriptionHelpFormatter)
-    ap.add_argument("--exp", required=True, choices=["table1", "exp1", "exp2", "ttest"])
+    ap.add_argument("--exp", required=True, choices=["table1", "exp1", "exp2", "ttest", "cfg2"])
     ap.add_argument("--seeds", type=int, default=0, help="seeds / instances (0: the paper's count)")
     a = ap.parse_args(argv)
     if a.exp == "table1":
@@ -140,6 +179,8 @@ def main(argv=None):
         rows = exp1(a.seeds or 20)
     elif a.exp == "exp2":
         rows = exp2(a.seeds or 20)
+    elif a.exp == "cfg2":
+        rows = cfg2()
     else:
         rows = ttest(a.seeds or 100)
     for r in rows:
