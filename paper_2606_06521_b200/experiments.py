@@ -137,7 +137,7 @@ def delta_k(k: int = 4) -> float:
     m = np.linspace(-10.0, 10.0, 200001)
     phi = np.exp(-0.5 * m * m) / math.sqrt(2.0 * math.pi)
     Phi = 0.5 * (1.0 + np.vectorize(math.erf)(m / math.sqrt(2.0)))
-    return float(np.trapz(m * k * phi * Phi ** (k - 1), m))
+    return float(np.trapezoid(m * k * phi * Phi ** (k - 1), m))
 
 
 def eq7(delta: float, S: float, k_sink: int = 4) -> float:
