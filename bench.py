@@ -7,8 +7,8 @@
 A step is one fp8attn_fwd call (the whole hot path: staging, QK^T, online softmax, P-cast,
 P.V, epilogue; plus the combine kernel for split-KV decode) over one synthetic batch of the
 named BASELINE.json config.  Default workload: cfg3 (configs[2]), the configuration the
-"FP8 attn fwd TFLOPS" metric is quoted on; cfg5 (decode, GB/s) is measured beside it and
-reported under "extra" unless --no-extra.
+"FP8 attn fwd TFLOPS" metric is quoted on; cfg4 in FP8 mode, cfg4 in BF16 isolation mode and cfg5
+(decode, GB/s) are measured beside it and reported under "extra" unless --no-extra.
 
 `value` is device-timed with inputs resident in HBM; `e2e` goes through fp8attn_fwd_host with
 pinned host buffers (H2D of q,k,v and D2H of o inside the timed region).  `--impl reference`
@@ -43,13 +43,20 @@ WORKLOADS = {
 
 
 def load_peaks():
-    """Measured peaks (driver-written MEASURED_PEAKS.json) or the profiling guide's fallback."""
+    """Measured peaks (driver-written MEASURED_PEAKS.json) or the profiling guide's fallback, plus the dense FP8
+    GEMM peak measured on this pool in round 2 (profiles/fp8_peak.json; SURVEY.md 8(d) "FP8 peak -- measure")."""
     p = os.path.join(ROOT, "MEASURED_PEAKS.json")
     if os.path.exists(p):
         m = json.load(open(p))
-        return {"hbm_gbs": m["hbm_gbs"], "bf16_tflops": m["bf16_tflops"],
-                "bf16_tflops_sustained": m.get("bf16_tflops_sustained", m["bf16_tflops"]), "source": "measured"}
-    return {"hbm_gbs": 6650.0, "bf16_tflops": 1590.0, "bf16_tflops_sustained": 1400.0, "source": "fallback"}
+        out = {"hbm_gbs": m["hbm_gbs"], "bf16_tflops": m["bf16_tflops"],
+               "bf16_tflops_sustained": m.get("bf16_tflops_sustained", m["bf16_tflops"]), "source": "measured"}
+    else:
+        out = {"hbm_gbs": 6650.0, "bf16_tflops": 1590.0, "bf16_tflops_sustained": 1400.0, "source": "fallback"}
+    try:
+        out["fp8"] = json.load(open(os.path.join(ROOT, "profiles", "fp8_peak.json")))
+    except (OSError, ValueError):
+        out["fp8"] = None
+    return out
 
 
 def ncu_traffic(workload, kernel):
@@ -65,62 +72,94 @@ def ncu_traffic(workload, kernel):
 
 # --------------------------------------------------------------------------- clocks
 class ClockSampler:
-    """nvidia-smi clock / throttle-reason samples during the timed region."""
+    """SM clock / throttle-reason samples while the GPU is under load: NVML every 5 ms from a thread (falls back to
+    an `nvidia-smi -lms 20` child process).  mark_start / mark_end bracket the timed region; the summary covers the
+    samples taken between them (`samples`) and says how many of those fell inside the CUDA-event-timed steps."""
     Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
          "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
          "clocks_event_reasons.sw_power_cap")
 
     def __init__(self, index):
-        self.index, self.proc, self.lines = index, None, []
-        self.lo = self.hi = None
+        self.index, self.proc, self.samples = index, None, []     # (t, sm_mhz, max_mhz, reasons)
+        self.t_lo = self.t_hi = None
+        self.stop = False
+        self.nvml = None
 
-    def mark_start(self):
-        """Timed region starts: wait for the sampler's first line (nvidia-smi takes a moment to come up)."""
-        t0 = time.time()
-        while self.proc and not self.lines and time.time() - t0 < 3.0:
-            time.sleep(0.01)
-        self.lo = len(self.lines)
+    def _nvml_loop(self):
+        n = self.nvml
+        h = n.nvmlDeviceGetHandleByIndex(self.index)
+        mx = float(n.nvmlDeviceGetMaxClockInfo(h, n.NVML_CLOCK_SM))
+        bits = {"hw_slowdown": n.nvmlClocksEventReasonHwSlowdown, "hw_thermal_slowdown": n.nvmlClocksEventReasonHwThermalSlowdown,
+                "sw_thermal_slowdown": n.nvmlClocksEventReasonSwThermalSlowdown, "sw_power_cap": n.nvmlClocksEventReasonSwPowerCap}
+        while not self.stop:
+            try:
+                sm = float(n.nvmlDeviceGetClockInfo(h, n.NVML_CLOCK_SM))
+                r = n.nvmlDeviceGetCurrentClocksEventReasons(h)
+                self.samples.append((time.time(), sm, mx, tuple(k for k, b in bits.items() if r & b)))
+            except Exception:
+                pass
+            time.sleep(0.005)
 
-    def mark_end(self):
-        time.sleep(0.06)
-        self.hi = len(self.lines)
-
-    def __enter__(self):
-        try:
-            self.proc = subprocess.Popen(["nvidia-smi", "-i", str(self.index), f"--query-gpu={self.Q}",
-                                          "--format=csv,noheader,nounits", "-lms", "50"],
-                                         stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
-            self.t = threading.Thread(target=lambda: self.lines.extend(self.proc.stdout), daemon=True)
-            self.t.start()
-        except OSError:
-            self.proc = None
-        return self
-
-    def __exit__(self, *a):
-        if self.proc:
-            time.sleep(0.06)
-            self.proc.terminate()
-            self.t.join(timeout=2)
-
-    def summary(self):
-        sm, mx, reasons = [], [], set()
+    def _smi_loop(self):
         names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
-        lines = self.lines[self.lo:self.hi] if self.lo is not None and self.hi is not None else self.lines
-        for ln in lines:
+        for ln in self.proc.stdout:
             f = [x.strip() for x in ln.split(",")]
             if len(f) < 7:
                 continue
             try:
-                sm.append(float(f[0])); mx.append(float(f[1]))
+                self.samples.append((time.time(), float(f[0]), float(f[1]),
+                                     tuple(n for n, val in zip(names, f[3:7]) if val.lower().startswith("active"))))
             except ValueError:
                 continue
-            for n, val in zip(names, f[3:7]):
-                if val.lower().startswith("active"):
-                    reasons.add(n)
-        if not sm:
+
+    def __enter__(self):
+        try:
+            import pynvml
+            pynvml.nvmlInit()
+            self.nvml = pynvml
+            self.t = threading.Thread(target=self._nvml_loop, daemon=True)
+            self.t.start()
+        except Exception:
+            self.nvml = None
+            try:
+                self.proc = subprocess.Popen(["nvidia-smi", "-i", str(self.index), f"--query-gpu={self.Q}",
+                                              "--format=csv,noheader,nounits", "-lms", "20"],
+                                             stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+                self.t = threading.Thread(target=self._smi_loop, daemon=True)
+                self.t.start()
+            except OSError:
+                self.proc = None
+        return self
+
+    def mark_start(self):
+        """Load starts: wait for the sampler's first sample (nvidia-smi takes a moment to come up)."""
+        t0 = time.time()
+        while (self.nvml or self.proc) and not self.samples and time.time() - t0 < 3.0:
+            time.sleep(0.005)
+        self.t_lo = time.time()
+
+    def mark_end(self):
+        self.t_hi = time.time()
+
+    def __exit__(self, *a):
+        self.stop = True
+        if self.proc:
+            time.sleep(0.05)
+            self.proc.terminate()
+        if self.nvml or self.proc:
+            self.t.join(timeout=2)
+
+    def summary(self, timed=None):
+        """timed = (t0, t1): wall-clock window of the CUDA-event-timed steps, counted separately."""
+        sel = [x for x in self.samples if self.t_lo is None or (self.t_lo <= x[0] <= (self.t_hi or x[0]))]
+        if not sel:
             return {"sm_mhz": None, "sm_max_mhz": None, "reasons": [], "samples": 0}
-        return {"sm_mhz": float(np.median(sm)), "sm_max_mhz": float(max(mx)), "reasons": sorted(reasons),
-                "samples": len(sm)}
+        reasons = sorted({r for x in sel for r in x[3]})
+        out = {"sm_mhz": float(np.median([x[1] for x in sel])), "sm_max_mhz": float(max(x[2] for x in sel)),
+               "reasons": reasons, "samples": len(sel), "source": "nvml 5 ms" if self.nvml else "nvidia-smi -lms 20"}
+        if timed is not None:
+            out["samples_in_timed_steps"] = sum(1 for x in sel if timed[0] <= x[0] <= timed[1])
+        return out
 
 
 # --------------------------------------------------------------------------- workload
@@ -168,6 +207,69 @@ def build_device_workload(cfg, kind, seed, dev):
     return q, k, v, sc
 
 
+def timed_steps(step, steps, warmup, dev, world=1, min_load_s=0.5):
+    """`warmup` untimed steps, then exactly `steps` steps timed with CUDA events on the current stream between
+    synchronisations (a barrier before, for N > 1).  The clock sampler runs from the first timed step on; if the
+    timed region is shorter than `min_load_s`, the same step keeps running (untimed) until then, so that the clock
+    record holds enough samples under the same load.  Returns (per-step ms, total ms, clocks, last result)."""
+    import torch
+    import torch.distributed as dist
+    with ClockSampler(dev.index or 0) as clk:
+        for _ in range(max(warmup, 3)):
+            r = step()
+        torch.cuda.synchronize()
+        if world > 1:
+            dist.barrier()
+        ev = [torch.cuda.Event(enable_timing=True) for _ in range(steps + 1)]
+        torch.cuda.synchronize()
+        clk.mark_start()
+        t0 = time.time()
+        ev[0].record()
+        for i in range(steps):
+            r = step()
+            ev[i + 1].record()
+        torch.cuda.synchronize()
+        t1 = time.time()
+        while time.time() - t0 < min_load_s:
+            for _ in range(8):
+                step()
+            torch.cuda.synchronize()
+        clk.mark_end()
+    per_step = [ev[i].elapsed_time(ev[i + 1]) for i in range(steps)]
+    return per_step, ev[0].elapsed_time(ev[steps]), clk.summary(timed=(t0, t1)), r
+
+
+def roofline_of(workload, cfg, mode, bound, amount, kern_ms, kernel_id, peaks):
+    """The roofline object of one workload: achieved = algorithmic FLOP (or bytes) per launch / measured launch time;
+    peak = the measured number for a kernel timed on its own (burst), the sustained one and my own FP8 GEMM
+    measurement beside it."""
+    if bound == "tensor":
+        is_fp8 = mode == 2
+        mult = 2.0 if is_fp8 else 1.0
+        roof = {"bound": "tensor", "achieved": amount / (kern_ms * 1e-3), "peak": peaks["bf16_tflops"] * mult, "unit": "TFLOP/s",
+                "peak_source": f"{peaks['source']} cuBLAS bf16 burst {peaks['bf16_tflops']} TFLOP/s"
+                               + (" x2 (guide's nominal fp8:bf16 ratio)" if is_fp8 else "")
+                               + "; burst, not sustained: the kernel is timed on its own at full clocks",
+                "peak_sustained": peaks["bf16_tflops_sustained"] * mult}
+        roof["frac_vs_sustained"] = roof["achieved"] / roof["peak_sustained"]
+        fp8 = peaks.get("fp8")
+        if is_fp8 and fp8:
+            roof["peak_measured_fp8"] = fp8["fp8_burst_tflops"]
+            roof["frac_vs_measured_fp8"] = roof["achieved"] / fp8["fp8_burst_tflops"]
+            roof["frac_vs_measured_fp8_sustained"] = roof["achieved"] / fp8["fp8_sustained_tflops"]
+            roof["peak_measured_fp8_source"] = fp8["how"]
+    else:
+        roof = {"bound": "hbm", "achieved": amount / (kern_ms * 1e-3), "peak": peaks["hbm_gbs"], "unit": "GB/s",
+                "peak_source": f"{peaks['source']} copy bandwidth (half reads, half writes; a read-only stream can "
+                               "exceed it, so frac may pass 1)",
+                "frac_vs_nominal_8000": amount / (kern_ms * 1e-3) / 8000.0}
+    roof["frac"] = roof["achieved"] / roof["peak"]
+    roof["kernel_ms"] = kern_ms
+    roof["kernel"] = {1: "attn_general_kernel", 2: "attn_prefill_kernel", 3: "attn_decode_kernel"}.get(kernel_id, "?")
+    roof["traffic"] = ncu_traffic(workload, roof["kernel"])
+    return roof
+
+
 def run_ours(args, rank, world, dev):
     import torch
     import torch.distributed as dist
@@ -182,26 +284,9 @@ def run_ours(args, rank, world, dev):
     def step():
         return fa.fwd(q, k, v, causal=cfg.causal, S=S, kv_order=order, mode=mode, out=o, **sc)
 
-    with ClockSampler(dev.index or 0) as clk:
-        for _ in range(max(args.warmup, 3)):
-            r = step()
-        torch.cuda.synchronize()
-        if world > 1:
-            dist.barrier()
-        ev = [torch.cuda.Event(enable_timing=True) for _ in range(args.steps + 1)]
-        torch.cuda.synchronize()
-        clk.mark_start()
-        ev[0].record()
-        for i in range(args.steps):
-            step()
-            ev[i + 1].record()
-        torch.cuda.synchronize()
-        clk.mark_end()
+    per_step, total_ms, clocks, r = timed_steps(step, args.steps, args.warmup, dev, world)
     if world > 1:
         dist.barrier()
-    per_step = [ev[i].elapsed_time(ev[i + 1]) for i in range(args.steps)]
-    total_ms = ev[0].elapsed_time(ev[args.steps])
-    if world > 1:
         t = torch.tensor([total_ms], dtype=torch.float64, device=dev)
         dist.all_reduce(t, op=dist.ReduceOp.MAX)
         total_ms = float(t.item())
@@ -261,20 +346,7 @@ def run_ours(args, rank, world, dev):
         del rs
 
     kern_ms = float(np.mean(per_step))
-    if bound == "tensor":
-        is_fp8 = mode == 2
-        peak = peaks["bf16_tflops"] * (2.0 if is_fp8 else 1.0)
-        roof = {"bound": "tensor", "achieved": amount / (kern_ms * 1e-3), "peak": peak, "unit": "TFLOP/s",
-                "peak_source": f"{peaks['source']} cuBLAS bf16 burst {peaks['bf16_tflops']} TFLOP/s"
-                               + (" x2 (guide's nominal fp8:bf16 ratio)" if is_fp8 else ""),
-                "peak_sustained": peaks["bf16_tflops_sustained"] * (2.0 if is_fp8 else 1.0)}
-    else:
-        roof = {"bound": "hbm", "achieved": amount / (kern_ms * 1e-3), "peak": peaks["hbm_gbs"], "unit": "GB/s",
-                "peak_source": f"{peaks['source']} copy bandwidth"}
-    roof["frac"] = roof["achieved"] / roof["peak"]
-    roof["kernel_ms"] = kern_ms
-    roof["kernel"] = {1: "attn_general_kernel", 2: "attn_prefill4_kernel", 3: "attn_decode_kernel"}.get(r.kernel_id, "?")
-    roof["traffic"] = ncu_traffic(args.workload, roof["kernel"])
+    roof = roofline_of(args.workload, cfg, mode, bound, amount, kern_ms, r.kernel_id, peaks)
     line = {
         "metric": "FP8 attention forward throughput" if bound == "tensor" else "split-KV decode attention bandwidth",
         "value": value, "unit": unit, "n_gpus": world, "steps": args.steps, "warmup": max(args.warmup, 3),
@@ -286,7 +358,7 @@ def run_ours(args, rank, world, dev):
                                f"mode={mode} inputs={kind}",
                    "block_m": r.block_m, "block_n": r.block_n, "num_splits": r.num_splits,
                    "l2": "inputs larger than L2 (no flush)", "sharding": "one replica of the workload per GPU"},
-        "clocks": clk.summary(), "e2e": e2e, "gpu_launches": int(r.n_launches * args.steps),
+        "clocks": clocks, "e2e": e2e, "gpu_launches": int(r.n_launches * args.steps),
         "roofline": roof,
     }
     if stats_cost is not None:
@@ -414,7 +486,7 @@ def main():
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--workload", choices=sorted(WORKLOADS), default="cfg3")
     ap.add_argument("--impl", choices=["ours", "reference"], default="ours")
-    ap.add_argument("--no-extra", action="store_true", help="skip the cfg5 decode measurement and the CPU baseline")
+    ap.add_argument("--no-extra", action="store_true", help="skip the other configs and the CPU baseline")
     args = ap.parse_args()
     rank = int(os.environ.get("RANK", "0"))
     local = int(os.environ.get("LOCAL_RANK", "0"))
@@ -438,13 +510,16 @@ def main():
     line = run_ours(args, rank, world, dev)
     if rank == 0 and not args.no_extra and world == 1:
         line["cpu_baseline"] = cpu_baseline(args.workload, line["unit"])
-        other = "cfg5" if args.workload != "cfg5" else "cfg3"
-        sub = argparse.Namespace(**{**vars(args), "workload": other, "steps": min(args.steps, 10)})
-        try:
-            ex = run_ours_extra(sub, dev)
-        except Exception as e:      # the extra measurement never takes the headline down
-            ex = {"error": repr(e)}
-        line["extra"] = {other: ex}
+        # every other BASELINE throughput config beside the headline, each with its own roofline and clock record
+        line["extra"] = {}
+        for other in ("cfg3", "cfg4-fp8", "cfg4-bf16", "cfg5"):
+            if other == args.workload:
+                continue
+            sub = argparse.Namespace(**{**vars(args), "workload": other, "steps": min(args.steps, 20)})
+            try:
+                line["extra"][other] = run_ours_extra(sub, dev)
+            except Exception as e:      # an extra measurement never takes the headline down
+                line["extra"][other] = {"error": repr(e)}
     if rank == 0:
         print(json.dumps(line), flush=True)
     if world > 1:
@@ -455,6 +530,8 @@ def main():
 
 
 def run_ours_extra(args, dev):
+    """One more workload measured the same way as the headline (device-resident inputs, CUDA events, clocks under
+    the same load), without the end-to-end and CPU legs."""
     import torch
     from paper_2606_06521_b200 import fp8attn as fa
     cfg_name, kind, mode, S, order = WORKLOADS[args.workload]
@@ -462,23 +539,40 @@ def run_ours_extra(args, dev):
     q, k, v, sc = build_device_workload(cfg, kind, seed=0, dev=dev)
     o = torch.empty((cfg.B, cfg.Hq, cfg.Lq, cfg.d), dtype=torch.float32, device=dev)
     amount, unit, bound = units(cfg, kind)
-    for _ in range(3):
-        r = fa.fwd(q, k, v, causal=cfg.causal, S=S, kv_order=order, mode=mode, out=o, **sc)
-    torch.cuda.synchronize()
-    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-    e0.record()
-    for _ in range(args.steps):
-        fa.fwd(q, k, v, causal=cfg.causal, S=S, kv_order=order, mode=mode, out=o, **sc)
-    e1.record()
-    torch.cuda.synchronize()
-    ms = e0.elapsed_time(e1) / args.steps
-    peaks = load_peaks()
-    peak = peaks["hbm_gbs"] if bound == "hbm" else peaks["bf16_tflops"] * (2.0 if mode == 2 else 1.0)
-    val = amount / (ms * 1e-3)
-    return {"value": val, "unit": unit, "ms_per_step": ms, "steps": args.steps, "kernel_id": r.kernel_id,
-            "num_splits": r.num_splits, "block_n": r.block_n, "gpu_launches_per_step": r.n_launches,
-            "roofline": {"bound": bound, "achieved": val, "peak": peak, "frac": val / peak,
-                         "unit": unit, "traffic": None}}
+
+    def step():
+        return fa.fwd(q, k, v, causal=cfg.causal, S=S, kv_order=order, mode=mode, out=o, **sc)
+
+    per_step, total_ms, clocks, r = timed_steps(step, args.steps, 3, dev)
+    ms = total_ms / args.steps
+    out = {"value": amount / (ms * 1e-3), "unit": unit, "ms_per_step": ms, "steps": args.steps, "kernel_id": r.kernel_id,
+           "num_splits": r.num_splits, "block_n": r.block_n, "gpu_launches_per_step": r.n_launches,
+           "dtype": "e4m3 (fp32 accumulate)" if mode == 2 else "bf16 (fp32 accumulate), P cast to e4m3",
+           "config": {"workload": f"{args.workload}: B={cfg.B} Hq={cfg.Hq} Hkv={cfg.Hkv} Lq={cfg.Lq} Lk={cfg.Lk} d={cfg.d} "
+                                  f"causal={cfg.causal} Delta={cfg.delta} S={S} order={'reverse' if order else 'forward'} "
+                                  f"mode={mode} inputs={kind}"},
+           "clocks": clocks,
+           "roofline": roofline_of(args.workload, cfg, mode, bound, amount, float(np.mean(per_step)), r.kernel_id,
+                                   load_peaks())}
+    if cfg.name == "cfg5":
+        # the same launch with the statistics instance of the decode kernel (P dump off, both underflow counters on)
+        def sstep():
+            return fa.fwd(q, k, v, causal=cfg.causal, S=S, kv_order=order, mode=mode, out=o, want_stats=True, **sc)
+        rs = sstep()
+        torch.cuda.synchronize()
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record()
+        for _ in range(10):
+            rs = sstep()
+        e1.record()
+        torch.cuda.synchronize()
+        uf = [int(x) for x in rs.underflow.cpu()]
+        out["with_statistics"] = {"ms_per_step": e0.elapsed_time(e1) / 10, "kernel_id": rs.kernel_id,
+                                  "value": amount / (e0.elapsed_time(e1) / 10 * 1e-3), "unit": unit,
+                                  "underflow_sink_block": uf[0], "underflow_other_blocks": uf[1]}
+    del q, k, v, o
+    torch.cuda.empty_cache()
+    return out
 
 
 if __name__ == "__main__":
