@@ -22,7 +22,14 @@
  * Parity pins (tests/test_oracle_*.py): E4M3 enumeration, RNE ties, dp(S) App. A
  * values, Prop. 5, no-cast == brute-force softmax, Table 1 / Eq. 7 underflow
  * fractions, Thm 4 zero-underflow.  "Parity unpinned by the paper" (pinned by
- * invariants only): split-KV + combine, per-(b,h) absmax/448 input quantisation.
+ * invariants only): split-KV + combine, per-(b,h) absmax/448 input quantisation,
+ * the dynamic per-block power-of-two scale (PAPER.md:435 names it as future work
+ * without a rule; reading R26, pinned by: equal to static 256 bit for bit when the
+ * exponent is constant, never an underflow that static 256 does not have, an
+ * independent offline recomputation), sink keys at arbitrary positions and the
+ * "sink blocks last" order (reading R27, pinned by: the prefix
+ * layout reproduces the default counters, zero underflow outside the sink blocks
+ * for S = 256, an independent offline recomputation).
  *
  * Arithmetic: FP64 everywhere except where Alg. 1 fixes FP32 (the logits Z, the
  * probabilities P, the product P*S and the running max are FP32 values).
@@ -207,7 +214,59 @@ typedef struct {
     uint64_t uf_other_blocks;/* out: total underflows elsewhere */
     uint64_t n_nonsink_visible; /* out: number of visible non-sink (row,key) pairs */
     int32_t n_threads;       /* 0 = OpenMP default; out: threads used */
+    int32_t scale_mode;      /* 0: static S (Alg. 1); 1: per-(row, block) power-of-two scale
+                                S_j = 2^k_j (reading R26), S is not used */
+    const int32_t *sink_pos; /* n_sink key indices (ascending) of the sink keys, or NULL: the
+                                first n_sink keys (reading R27) */
 } fp8attn_oracle_opts;
+
+/* Largest exponent the dynamic scale takes (reading R26). */
+#define DYN_K_MAX 30
+
+static int is_sink_key(const fp8attn_oracle_opts *o, int j)
+{
+    if (!o->sink_pos)
+        return j < o->n_sink;
+    for (int s = 0; s < o->n_sink; ++s)
+        if (o->sink_pos[s] == j)
+            return 1;
+    return 0;
+}
+
+/* Does block [j0, j0 + Bn) hold a sink key? */
+static int is_sink_block(const fp8attn_oracle_opts *o, int j0, int Bn)
+{
+    if (!o->sink_pos)
+        return j0 < o->n_sink;
+    for (int s = 0; s < o->n_sink; ++s)
+        if (o->sink_pos[s] >= j0 && o->sink_pos[s] < j0 + Bn)
+            return 1;
+    return 0;
+}
+
+/*
+ * Block visited at step `step` of the range [b0, b1) (Alg. 1 line 2).
+ *   order 0: forward b0 .. b1-1.   order 1: reverse b1-1 .. b0.
+ *   order 2: "sink blocks last" (reading R27): the blocks that hold no sink
+ *            key in descending order, then the blocks that hold one, in descending order.
+ *            With the sink keys in block 0 this is order 1.
+ */
+static int block_at(const fp8attn_oracle_opts *o, int order, int b0, int b1, int step, int Bn)
+{
+    if (order == 0)
+        return b0 + step;
+    if (order == 1)
+        return b1 - 1 - step;
+    int seen = 0;
+    for (int pass = 0; pass < 2; ++pass)          /* pass 0: non-sink blocks, pass 1: sink blocks */
+        for (int b = b1 - 1; b >= b0; --b)
+            if (is_sink_block(o, b * Bn, Bn) == pass) {
+                if (seen == step)
+                    return b;
+                ++seen;
+            }
+    return -1;
+}
 
 typedef struct {
     const void *q, *k, *v;
@@ -325,7 +384,7 @@ static void attend_row(const problem *P, int64_t rid, int64_t sel,
         double l = 0.0;
         double *O = Os + (size_t)s * d;
         for (int step = 0; step < b1 - b0; ++step) {
-            int blk = (P->kv_order == 0) ? b0 + step : b1 - 1 - step;   /* line 2 */
+            int blk = block_at(o, P->kv_order, b0, b1, step, Bn);       /* line 2 */
             int j0 = blk * Bn;
             int j1 = j0 + Bn < Lk ? j0 + Bn : Lk;
             if (j1 - 1 > jmax) j1 = jmax + 1;
@@ -336,7 +395,20 @@ static void attend_row(const problem *P, int64_t rid, int64_t sel,
             double alpha = isinf(m) ? 0.0 : exp((double)m - (double)m_new);   /* line 6 */
             double psum = 0.0;
             for (int t = 0; t < d; ++t) O[t] *= alpha;
-            int sink_blk = (j0 < o->n_sink);
+            int sink_blk = is_sink_block(o, j0, Bn);
+            /* scale of this block.  Static: S.  Dynamic (reading R26): the largest power of two
+             * 2^k with 2^k * max_j p_j <= 448, where max_j p_j = exp(m_loc - m_new); taken in FP32
+             * in base-2 units, k = floor(log2(448) + (m_new - m_loc) log2(e)), capped at DYN_K_MAX.
+             * O then holds true (unscaled) values: each block's contribution is divided by its own
+             * 2^k, which is exact (Prop. 5). */
+            float Sblk = Sf;
+            if (o->scale_mode == 1 && P->mode != 0) {
+                float g2 = (m_new - m_loc) * 1.44269504088896340736f;
+                int kexp = (int)floorf(g2 + 8.80735492205760410744f);
+                if (kexp > DYN_K_MAX) kexp = DYN_K_MAX;
+                Sblk = ldexpf(1.0f, kexp);
+            }
+            const double Sblk_d = (o->scale_mode == 1 && P->mode != 0) ? (double)Sblk : 1.0;
             for (int j = j0; j < j1; ++j) {
                 float p = (float)exp((double)z[j] - (double)m_new);           /* line 7 */
                 psum += (double)p;
@@ -344,11 +416,11 @@ static void attend_row(const problem *P, int64_t rid, int64_t sel,
                 if (P->mode == 0) {
                     pq = (double)p;                /* no-cast reference */
                 } else {
-                    float x = p * Sf;              /* line 9: xS in FP32 */
+                    float x = p * Sblk;            /* line 9: xS in FP32 */
                     uint8_t c = fp8attn_oracle_round_e4m3(x);
-                    pq = e4m3_code_value(c);
+                    pq = e4m3_code_value(c) / Sblk_d;
                     if (codes_out) codes_out[j] = c;
-                    if (j >= o->n_sink) {
+                    if (!is_sink_key(o, j)) {
                         ++my_vis;
                         if (c == 0) { if (sink_blk) ++my_sink; else ++my_other; }
                     }
@@ -375,7 +447,7 @@ static void attend_row(const problem *P, int64_t rid, int64_t sel,
         for (int t = 0; t < d; ++t) out[t] += w * Os[(size_t)s * d + t];
     }
     if (lfin > 0.0)
-        for (int t = 0; t < d; ++t) out[t] /= (Sd * lfin);
+        for (int t = 0; t < d; ++t) out[t] /= ((o->scale_mode == 1 ? 1.0 : Sd) * lfin);
     if (o->row_max) o->row_max[sel] = mfin;
     if (o->row_sum) o->row_sum[sel] = lfin;
     if (o->row_uf_sink) o->row_uf_sink[sel] = my_sink;
@@ -401,7 +473,8 @@ ORACLE_API int fp8attn_oracle_fwd(const void *q, const void *k, const void *v, d
     if (B < 1 || Hq < 1 || Hkv < 1 || Lq < 1 || Lk < 1 || d < 1) return -2;
     if (Hq % Hkv) return -3;
     if (!(S > 0.0f) || isinf(S)) return -4;
-    if (mode < 0 || mode > 2 || (kv_order != 0 && kv_order != 1)) return -5;
+    if (mode < 0 || mode > 2 || kv_order < 0 || kv_order > 2) return -5;
+    if (opts->scale_mode != 0 && opts->scale_mode != 1) return -5;
     if (opts->block_n < 1 || opts->in_dtype < 0 || opts->in_dtype > 3) return -6;
     if ((opts->in_dtype == DT_E4M3 && (!opts->q_scale || !opts->k_scale || !opts->v_scale)) ||
         (opts->in_dtype == DT_BF16Q_E4M3KV && (!opts->k_scale || !opts->v_scale)))

@@ -24,6 +24,7 @@ class _Opts(C.Structure):
         ("p_codes", C.c_void_p), ("row_uf_sink", C.c_void_p), ("row_uf_other", C.c_void_p),
         ("uf_sink_block", C.c_uint64), ("uf_other_blocks", C.c_uint64),
         ("n_nonsink_visible", C.c_uint64), ("n_threads", C.c_int32),
+        ("scale_mode", C.c_int32), ("sink_pos", C.c_void_p),
     ]
 
 
@@ -126,9 +127,12 @@ def attention_fwd(q, k, v, *, causal: bool, S: float, kv_order: int, mode: int,
                   split_bounds: Optional[Sequence[int]] = None,
                   q_scale=None, k_scale=None, v_scale=None,
                   rows: Optional[Sequence[int]] = None, want_codes: bool = False,
-                  n_threads: int = 0) -> OracleResult:
+                  n_threads: int = 0, scale_mode: int = 0,
+                  sink_pos: Optional[Sequence[int]] = None) -> OracleResult:
     """q [B,Hq,Lq,d], k/v [B,Hkv,Lk,d] numpy arrays (float32, uint16 = BF16 bits, uint8 =
-    E4M3 codes).  Returns the cast-P output and statistics for the selected rows."""
+    E4M3 codes).  Returns the cast-P output and statistics for the selected rows.
+    kv_order 0 forward, 1 reverse, 2 sink blocks last; scale_mode 1 = dynamic per-(row, block) 2^k scale (S unused);
+    sink_pos = key indices of the sink keys (default: the first n_sink keys)."""
     q = _as_input(q, in_dtype, True)
     k = _as_input(k, in_dtype, False)
     v = _as_input(v, in_dtype, False)
@@ -169,6 +173,12 @@ def attention_fwd(q, k, v, *, causal: bool, S: float, kv_order: int, mode: int,
     o.p_codes = codes.ctypes.data if want_codes else None
     o.row_uf_sink, o.row_uf_other = ufs.ctypes.data, ufo.ctypes.data
     o.n_threads = n_threads
+    o.scale_mode = scale_mode
+    if sink_pos is not None:
+        sp = np.ascontiguousarray(sorted(int(x) for x in sink_pos), dtype=np.int32)
+        assert sp.size >= 1 and sp[0] >= 0 and sp[-1] < Lk and np.all(np.diff(sp) > 0)
+        keep.append(sp)
+        o.n_sink, o.sink_pos = int(sp.size), sp.ctypes.data
     rc = _load().fp8attn_oracle_fwd(q.ctypes.data, k.ctypes.data, v.ctypes.data, out.ctypes.data,
                                     B, Hq, Hkv, Lq, Lk, d, int(bool(causal)), float(S),
                                     int(kv_order), int(mode), C.byref(o))

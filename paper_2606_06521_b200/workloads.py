@@ -43,15 +43,18 @@ CONFIGS = {
 }
 
 
-def sink_qkv(B, Hq, Hkv, Lq, Lk, d, delta, n_sink=4, seed=0):
-    """FP32 Q [B,Hq,Lq,d], K, V [B,Hkv,Lk,d] with the sink construction."""
+def sink_qkv(B, Hq, Hkv, Lq, Lk, d, delta, n_sink=4, seed=0, sink_positions=None):
+    """FP32 Q [B,Hq,Lq,d], K, V [B,Hkv,Lk,d] with the sink construction.  `sink_positions` puts the sink keys at
+    the given key indices instead of the first n_sink (multi-sink / distributed-sink layouts); the
+    random draws do not depend on it."""
     rng = np.random.default_rng(seed)
     q = rng.standard_normal((B, Hq, Lq, d), dtype=np.float32)
     k = rng.standard_normal((B, Hkv, Lk, d), dtype=np.float32)
     v = rng.standard_normal((B, Hkv, Lk, d), dtype=np.float32)
     q[..., d - 1] = 1.0
     k[..., d - 1] = 0.0
-    k[..., :n_sink, d - 1] = np.float32(delta * np.sqrt(d))
+    pos = list(range(n_sink)) if sink_positions is None else [int(x) for x in sink_positions]
+    k[..., pos, d - 1] = np.float32(delta * np.sqrt(d))
     return q, k, v
 
 
