@@ -49,15 +49,35 @@ extern "C" {
 /* ---- `kv_order` ---------------------------------------------------------------------- */
 #define FP8ATTN_ORDER_FORWARD 0     /* blocks 0 .. nb-1                                          */
 #define FP8ATTN_ORDER_REVERSE 1     /* blocks nb-1 .. 0 (sink block last)          */
+#define FP8ATTN_ORDER_SINK_LAST 2   /* sink keys anywhere (stats->sink_pos): the blocks that hold no
+                                       sink key in descending order, then the blocks that hold one,
+                                       in descending order (the per-block view of PAPER.md:443;
+                                       DESIGN.md reading R27).  With the sink keys in block 0 this
+                                       is FP8ATTN_ORDER_REVERSE.  General and decode kernels.     */
+
+/* ---- stats->scale_mode --------------------------------------------------------------- */
+#define FP8ATTN_SCALE_STATIC  0     /* P * S, the static scale of Alg. 1 line 9                  */
+#define FP8ATTN_SCALE_DYNAMIC 1     /* per-(row, block) power-of-two scale S_j = 2^k_j, k_j the
+                                       largest k <= 30 with 2^k * exp(m_loc - m_new) <= 448, i.e.
+                                       k_j = floor(log2 448 + (m_new - m_loc) log2 e) in FP32
+                                       ("dynamic per-block scale ... constrained to
+                                       2^k"; reading R26).  S is not used.  Modes 1, 2;
+                                       general, decode and Bn = 128 prefill kernels.             */
+
+/* ---- stats->o_dtype ------------------------------------------------------------------ */
+#define FP8ATTN_O_F32  0
+#define FP8ATTN_O_BF16 1            /* o is bfloat16 (round to nearest even in the epilogue)      */
+
+#define FP8ATTN_MAX_SINKS 32
 
 /* ---- error codes --------------------------------------------------------------------- */
 #define FP8ATTN_OK              0
 #define FP8ATTN_E_NULL         -1   /* a required pointer is NULL                                */
 #define FP8ATTN_E_SHAPE        -2   /* a size is < 1, Hq % Hkv != 0, or d not in {64, 128}       */
 #define FP8ATTN_E_SCALE        -3   /* S is not a finite FP32 > 0                                */
-#define FP8ATTN_E_MODE         -4   /* unknown mode / dtype / kv_order, or a combination that is
-                                       not defined (mode 2 needs E4M3 k,v; modes 0,1 need
-                                       FP32/BF16)                                               */
+#define FP8ATTN_E_MODE         -4   /* unknown mode / dtype / kv_order / scale_mode / o_dtype, or a
+                                       combination that is not defined (mode 2 needs E4M3 k,v;
+                                       modes 0,1 need FP32/BF16; the dynamic scale needs a cast)  */
 #define FP8ATTN_E_UNSUPPORTED  -5   /* valid but not built: E4M3 with d != 128 (a 64-byte operand
                                        row does not fill the 128-byte swizzle row the kernels are
                                        built on), block_n not in {0, 64, 128}, FP32 inputs with
@@ -76,8 +96,10 @@ extern "C" {
 typedef struct fp8attn_stats {
     /* ---- inputs ---- */
     int32_t struct_size;       /* sizeof(fp8attn_stats)                                          */
-    int32_t n_sink;            /* number of sink keys at the start of the sequence (k_sink,
-                                  PAPER.md:131); only used to classify underflows               */
+    int32_t n_sink;            /* number of sink keys (k_sink): the first n_sink keys
+                                  of the sequence, or the n_sink <= FP8ATTN_MAX_SINKS entries of
+                                  sink_pos.  Used to classify underflows and by
+                                  FP8ATTN_ORDER_SINK_LAST                                        */
     int32_t block_n;           /* KV block size Bn request: 0 = library default, else 64 or 128
                                   ("typically 64 or 128")                          */
     int32_t num_splits;        /* split-KV request: 0 = automatic, n >= 1 = exactly n contiguous
@@ -85,7 +107,7 @@ typedef struct fp8attn_stats {
     int32_t kernel;            /* kernel family request: 0 = automatic, 1 = general kernel, 2 = warp-
                                   specialised prefill kernel, 3 = split-KV decode kernel; a family
                                   that cannot serve the call gives FP8ATTN_E_UNSUPPORTED       */
-    int32_t reserved0;         /* must be 0                                                      */
+    int32_t scale_mode;        /* FP8ATTN_SCALE_*                                                */
     const float *q_scale;      /* device [B*Hq]  dequantisation scale of E4M3 q (value = code*scale) */
     const float *k_scale;      /* device [B*Hkv]                                                 */
     const float *v_scale;      /* device [B*Hkv]                                                 */
@@ -99,6 +121,10 @@ typedef struct fp8attn_stats {
                                   schedule as the throughput instance) and of the decode kernel
                                   (the automatic choice for decode shapes)                        */
     int32_t p_batch, p_head;
+    const int32_t *sink_pos;   /* HOST pointer or NULL: n_sink key indices, ascending, of the sink
+                                  keys (multi-sink / distributed-sink layouts)    */
+    int32_t o_dtype;           /* FP8ATTN_O_*                                                    */
+    int32_t reserved1;         /* must be 0                                                      */
     /* ---- outputs, device (each may be NULL) ---- */
     float *row_max;            /* [B,Hq,Lq] final running max m (scaled logits, natural log)    */
     float *row_sum;            /* [B,Hq,Lq] final l relative to m; NOT multiplied by S           */
@@ -119,7 +145,7 @@ typedef struct fp8attn_stats {
 
 /*
  * fp8attn_fwd -- attention forward (Alg. 1).
- *   q, o : device, [B, Hq, Lq, d] contiguous row-major; o is always float32.
+ *   q, o : device, [B, Hq, Lq, d] contiguous row-major; o is float32 (bfloat16 with stats->o_dtype).
  *   k, v : device, [B, Hkv, Lk, d]; query head h reads kv head h / (Hq / Hkv).
  *   d    : 64 or 128.  Softmax scale is 1/sqrt(d).
  *   causal : nonzero = key j visible to query i iff j <= i + (Lk - Lq) (bottom-right).

@@ -14,6 +14,7 @@
 // block, l from the FP32 pre-cast P, P*S cast with cvt.rn.satfinite.e4m3x2.f32, O / (S l) at the end (or in the
 // combine kernel when the KV range is split).
 #pragma once
+#include <cuda_bf16.h>
 #include "common.cuh"
 
 namespace fp8attn {
@@ -117,7 +118,7 @@ attn_decode_kernel(const __grid_constant__ CUtensorMap mapQ, const __grid_consta
             ptx::mbar_arrive_expect_tx(q_full, C::Q_BYTES);
             ptx::tma_load_3d(sQ, &mapQ, q_full, 0, (int)row0, 0);
             for (int it = 0; it < n_it; ++it) {
-                const int blk = (p.kv_order == 0) ? sb0 + it : sb1 - 1 - it;
+                const int blk = block_at(p, sb0, sb1, it, C::BN);
                 const int st = it % C::NS;
                 const uint32_t ph = (it / C::NS) & 1;
                 ptx::mbar_wait(k_empty + st, ph ^ 1);
@@ -186,6 +187,8 @@ attn_decode_kernel(const __grid_constant__ CUtensorMap mapQ, const __grid_consta
         const float c_nat = p.sm_scale * p.k_scale[kvslab];     // times q_scale[row] below (per query head)
         float cl2[NVT], m_run[NVT], l_t[NVT];
         int jlim[NVT];
+        int k_run[NVT];                  // dynamic scale: O^T column n and l_t[n] carry 2^k_run[n]
+        const bool dynamic = p.scale_mode == 1;
 #pragma unroll
         for (int n = 0; n < NVT; ++n) {
             const int g = n / p.Lq, lq = n % p.Lq;
@@ -193,6 +196,7 @@ attn_decode_kernel(const __grid_constant__ CUtensorMap mapQ, const __grid_consta
             cl2[n] = c_nat * qs * LOG2E;
             m_run[n] = -INFINITY;
             l_t[n] = 0.0f;
+            k_run[n] = 0;
             long long jl = p.causal ? (long long)lq + off : (long long)p.Lk - 1;
             if (jl > p.Lk - 1) jl = p.Lk - 1;
             jlim[n] = (n < nv) ? (int)jl : -1;
@@ -209,7 +213,7 @@ attn_decode_kernel(const __grid_constant__ CUtensorMap mapQ, const __grid_consta
         }
 
         for (int j = 0; j < n_it; ++j) {
-            const int blk = (p.kv_order == 0) ? sb0 + j : sb1 - 1 - j;
+            const int blk = block_at(p, sb0, sb1, j, C::BN);
             const int key = blk * C::BN + tid;
             const int buf = j & 1;
             ptx::mbar_wait(s_full + buf, (j >> 1) & 1);
@@ -243,10 +247,19 @@ attn_decode_kernel(const __grid_constant__ CUtensorMap mapQ, const __grid_consta
             for (int n = 0; n < NVT; ++n) {
                 const int* w = wmax + buf * 64 + n;
                 const int mi = max(max(w[0], w[16]), max(w[32], w[48]));
-                const float m_new = fmaxf(m_run[n], ordered_to_float(mi));
+                const float m_loc = ordered_to_float(mi);
+                const float m_new = fmaxf(m_run[n], m_loc);
                 const float m_used = (m_new == -INFINITY) ? 0.0f : m_new;
                 alpha[n] = ptx::ex2_approx((m_run[n] - m_used) * cl2[n]);    // line 6
                 negm[n] = fmaf(-m_used, cl2[n], log2S);
+                if (dynamic) {
+                    // reading R26: this block's scale 2^k goes into the exponent of P, and what O^T and l carry
+                    // (the previous block's scale) is brought to it together with alpha
+                    const int k_new = (m_loc == -INFINITY) ? k_run[n] : dyn_exponent((m_new - m_loc) * cl2[n]);
+                    negm[n] = fmaf(-m_used, cl2[n], (float)k_new);
+                    alpha[n] *= exp2f((float)(k_new - k_run[n]));
+                    k_run[n] = k_new;
+                }
                 any_rescale |= (n < nv) && (alpha[n] != 1.0f);
                 m_run[n] = m_new;
             }
@@ -260,7 +273,7 @@ attn_decode_kernel(const __grid_constant__ CUtensorMap mapQ, const __grid_consta
                 const float p1 = ptx::ex2_approx(fmaf(s[n + 1], cl2[n + 1], negm[n + 1]));
                 l_t[n] = alpha[n] * l_t[n] + p0;                              // line 8
                 l_t[n + 1] = alpha[n + 1] * l_t[n + 1] + p1;
-                const uint32_t pair = FOLD ? ptx::cvt_e4m3x2(p0, p1) : ptx::cvt_e4m3x2(p0 * p.S, p1 * p.S);   // line 9
+                const uint32_t pair = (FOLD || dynamic) ? ptx::cvt_e4m3x2(p0, p1) : ptx::cvt_e4m3x2(p0 * p.S, p1 * p.S);   // line 9
                 prow[n * 128 + ((chunk ^ (n & 7)) << 4)] = (uint8_t)(pair & 0xFFu);
                 prow[(n + 1) * 128 + ((chunk ^ ((n + 1) & 7)) << 4)] = (uint8_t)(pair >> 8);
                 if constexpr (AUX) {
@@ -272,8 +285,8 @@ attn_decode_kernel(const __grid_constant__ CUtensorMap mapQ, const __grid_consta
                         const bool vis = key <= jlim[nn];        // jlim = -1 for the padding rows nn >= nv
                         if (vis && dump_n0 >= 0 && nn >= dump_n0 && nn < dump_n0 + p.Lq)
                             p.p_codes[(size_t)(nn - dump_n0) * p.Lk + key] = (uint8_t)code;
-                        if (vis && key >= p.n_sink && code == 0u) {
-                            if (blk * C::BN < p.n_sink) ++uf_sink; else ++uf_other;
+                        if (vis && code == 0u && !is_sink_key(p, key)) {
+                            if (sink_in_range(p, blk * C::BN, C::BN)) ++uf_sink; else ++uf_other;
                         }
                     }
                 }
@@ -343,20 +356,24 @@ attn_decode_kernel(const __grid_constant__ CUtensorMap mapQ, const __grid_consta
 #pragma unroll
         for (int n = 0; n < NVT; ++n) {
             if (n >= nv) break;
-            const float l = (wsum[n] + wsum[16 + n]) + (wsum[32 + n] + wsum[48 + n]);   // carries S when FOLD
-            const float l_true = FOLD ? l / p.S : l;
+            const float l = (wsum[n] + wsum[16 + n]) + (wsum[32 + n] + wsum[48 + n]);   // carries S when FOLD / dynamic
+            const float carried = dynamic ? exp2f((float)k_run[n]) : (FOLD ? p.S : 1.0f);    // what l and O^T carry
+            const float l_true = l / carried;
             const float m_nat = (m_run[n] == -INFINITY) ? -INFINITY : m_run[n] * (cl2[n] / LOG2E);
             const long long grow = row0 + n;
             if (p.num_splits == 1) {
-                const float inv = (l > 0.0f) ? (FOLD ? vs / l : vs / (p.S * l)) : 0.0f;
-                p.o[grow * C::D + tid] = (l > 0.0f) ? __uint_as_float(ov[n]) * inv : 0.0f;
+                const float inv = (l > 0.0f) ? ((FOLD || dynamic) ? vs / l : vs / (p.S * l)) : 0.0f;
+                const float val = (l > 0.0f) ? __uint_as_float(ov[n]) * inv : 0.0f;
+                if (p.o_bf16) static_cast<__nv_bfloat16*>(p.o)[grow * C::D + tid] = __float2bfloat16_rn(val);
+                else static_cast<float*>(p.o)[grow * C::D + tid] = val;
                 if (tid == 0) {
                     if (p.row_max) p.row_max[grow] = m_nat;
                     if (p.row_sum) p.row_sum[grow] = l_true;
                 }
             } else {
-                // unnormalised partial: O (carrying S like the general kernel's partials), m, l
-                p.part_o[((long long)split * R + grow) * C::D + tid] = __uint_as_float(ov[n]);
+                // unnormalised partial: O carrying S like the general kernel's partials (dynamic: true units), m, l
+                p.part_o[((long long)split * R + grow) * C::D + tid] =
+                    dynamic ? __uint_as_float(ov[n]) / carried : __uint_as_float(ov[n]);
                 if (tid == 0) {
                     p.part_ml[((long long)split * R + grow) * 2 + 0] = m_nat;
                     p.part_ml[((long long)split * R + grow) * 2 + 1] = l_true;

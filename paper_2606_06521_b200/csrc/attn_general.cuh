@@ -11,6 +11,7 @@
 // no-cast mode, P-code dump, underflow counters, split-KV partials); the throughput kernels
 // live in attn_prefill.cuh / attn_prefill64.cuh / attn_decode.cuh.
 #pragma once
+#include <cuda_bf16.h>
 #include "common.cuh"
 
 namespace fp8attn {
@@ -118,6 +119,8 @@ attn_general_kernel(const __grid_constant__ CUtensorMap mapQ, const __grid_const
     }
 
     float m_run = -INFINITY, l_run = 0.0f;
+    int k_run = 0;            // dynamic scale: O in TMEM carries 2^k_run (the exponent of the last block)
+    const bool dynamic = (MODE != 0) && p.scale_mode == 1;
     unsigned int uf_sink = 0, uf_other = 0;
     const bool dump = (MODE != 0) && p.p_codes != nullptr && bh == p.p_bh && qrow < p.Lq;
     const bool count = (MODE != 0) && p.underflow != nullptr && qrow < p.Lq;
@@ -127,7 +130,7 @@ attn_general_kernel(const __grid_constant__ CUtensorMap mapQ, const __grid_const
     constexpr uint32_t idesc_pv = ptx::make_idesc(pfmt, C::FMT, ptx::MAJOR_K, ptx::MAJOR_MN, BM, D);
 
     for (int it = 0; it < n_iter; ++it) {
-        const int blk = (p.kv_order == 0) ? sb0 + it : blk_hi - 1 - it;
+        const int blk = block_at(p, sb0, blk_hi, it, BN);
         const int j0 = blk * BN;
         const uint32_t ph = it & 1;
 
@@ -185,7 +188,15 @@ attn_general_kernel(const __grid_constant__ CUtensorMap mapQ, const __grid_const
         const float m_used = (m_new == -INFINITY) ? 0.0f : m_new;
         const float alpha = ptx::ex2_approx((m_run - m_used) * cl2);   // line 6 (0 when m_run = -inf)
         const float neg_ml2 = -m_used * cl2;
-        const bool sink_blk = j0 < p.n_sink;
+        const bool sink_blk = sink_in_range(p, j0, BN);
+        // scale of this block: S, or (reading R26) the largest 2^k that keeps the block maximum at or below 448
+        float S_blk = S_eff, o_factor = alpha;          // o_factor: what O (carrying the previous scale) is multiplied by
+        if (dynamic) {
+            const int k_new = (mloc == -INFINITY) ? k_run : dyn_exponent((m_new - mloc) * cl2);
+            S_blk = exp2f((float)k_new);
+            o_factor = alpha * exp2f((float)(k_new - k_run));
+            k_run = k_new;
+        }
 
         // ---- lines 7-9: P, row sum from the pre-cast P, cast, P -> TMEM ----
         float psum = 0.0f;
@@ -220,14 +231,14 @@ attn_general_kernel(const __grid_constant__ CUtensorMap mapQ, const __grid_const
                 uint32_t pair[16];
 #pragma unroll
                 for (int e = 0; e < 32; e += 2)
-                    pair[e / 2] = ptx::cvt_e4m3x2(pr[e] * S_eff, pr[e + 1] * S_eff);   // line 9
+                    pair[e / 2] = ptx::cvt_e4m3x2(pr[e] * S_blk, pr[e + 1] * S_blk);   // line 9
                 if (count || dump) {
 #pragma unroll
                     for (int e = 0; e < 32; ++e) {
                         const int j = j0 + cb * 32 + e;
                         const uint32_t code = (pair[e / 2] >> ((e & 1) * 8)) & 0xFFu;
                         const bool vis = j <= jlim;
-                        if (count && vis && j >= p.n_sink && code == 0) {
+                        if (count && vis && code == 0 && !is_sink_key(p, j)) {
                             if (sink_blk) ++uf_sink; else ++uf_other;
                         }
                         if (dump && j < p.Lk) p.p_codes[(size_t)qrow * p.Lk + j] = vis ? (uint8_t)code : (uint8_t)0xFF;
@@ -262,7 +273,7 @@ attn_general_kernel(const __grid_constant__ CUtensorMap mapQ, const __grid_const
                 ptx::tmem_ld_x32(tlane + C::TM_O + cb * 32, v);
                 ptx::tmem_wait_ld();
 #pragma unroll
-                for (int e = 0; e < 32; ++e) v[e] = __float_as_uint(__uint_as_float(v[e]) * alpha);
+                for (int e = 0; e < 32; ++e) v[e] = __float_as_uint(__uint_as_float(v[e]) * o_factor);
                 ptx::tmem_st_x32(tlane + C::TM_O + cb * 32, v);
             }
         }
@@ -315,8 +326,10 @@ attn_general_kernel(const __grid_constant__ CUtensorMap mapQ, const __grid_const
             p.part_ml[((long long)split * R + grow) * 2 + 1] = l_run;
         }
     }
-    const float inv = (p.num_splits == 1) ? ((l_run > 0.0f) ? vs / (S_eff * l_run) : 0.0f) : 1.0f;
-    float* dst = (p.num_splits == 1) ? p.o + grow * D : p.part_o + ((long long)split * R + grow) * D;
+    // (dynamic scale: O carries 2^k_run; partials of a split are written in true units, the combine divides by 1)
+    const float S_fin = dynamic ? exp2f((float)k_run) : S_eff;
+    const float inv = (p.num_splits == 1) ? ((l_run > 0.0f) ? vs / (S_fin * l_run) : 0.0f) : (dynamic ? 1.0f / S_fin : 1.0f);
+    float* const dst_part = p.part_o + ((long long)split * R + grow) * D;
 #pragma unroll 1
     for (int cb = 0; cb < D / 32; ++cb) {
         uint32_t v[32];
@@ -336,7 +349,8 @@ attn_general_kernel(const __grid_constant__ CUtensorMap mapQ, const __grid_const
                 o4.z = __uint_as_float(v[e + 2]) * inv;
                 o4.w = __uint_as_float(v[e + 3]) * inv;
                 if (l_run <= 0.0f) o4 = make_float4(0.f, 0.f, 0.f, 0.f);
-                *reinterpret_cast<float4*>(dst + cb * 32 + e) = o4;
+                if (p.num_splits == 1) store_o4(p, grow * D + cb * 32 + e, o4.x, o4.y, o4.z, o4.w);
+                else *reinterpret_cast<float4*>(dst_part + cb * 32 + e) = o4;
             }
         }
     }
@@ -356,9 +370,9 @@ attn_general_kernel(const __grid_constant__ CUtensorMap mapQ, const __grid_const
 // ---------------------------------------------------------------------------------------------
 // Combine of split-KV partials: m = max_s m_s; w_s = exp(m_s - m);
 // O = sum_s w_s O_s / (S sum_s w_s l_s) (x v_scale in mode 2).  One warp per row.
-__global__ void combine_kernel(const float* __restrict__ part_o, const float* __restrict__ part_ml, float* __restrict__ o,
+__global__ void combine_kernel(const float* __restrict__ part_o, const float* __restrict__ part_ml, void* __restrict__ o,
                                float* __restrict__ row_max, float* __restrict__ row_sum, const float* __restrict__ v_scale,
-                               long long R, int d, int ns, float S_eff, int Hq, int Hkv, int Lq) {
+                               long long R, int d, int ns, float S_eff, int Hq, int Hkv, int Lq, int o_bf16) {
     const long long row = (long long)blockIdx.x * (blockDim.x / 32) + (threadIdx.x >> 5);
     const int lane = threadIdx.x & 31;
     if (row >= R) return;
@@ -380,7 +394,10 @@ __global__ void combine_kernel(const float* __restrict__ part_o, const float* __
         vs = v_scale[(bh / Hq) * Hkv + (bh % Hq) / (Hq / Hkv)];
     }
     const float inv = l > 0.0f ? vs / (S_eff * l) : 0.0f;
-    for (int t = lane, i = 0; t < d; t += 32, ++i) o[row * d + t] = acc[i] * inv;
+    for (int t = lane, i = 0; t < d; t += 32, ++i) {
+        if (o_bf16) static_cast<__nv_bfloat16*>(o)[row * d + t] = __float2bfloat16_rn(acc[i] * inv);
+        else static_cast<float*>(o)[row * d + t] = acc[i] * inv;
+    }
     if (lane == 0) {
         if (row_max) row_max[row] = m;
         if (row_sum) row_sum[row] = l;

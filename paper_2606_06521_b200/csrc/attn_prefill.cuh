@@ -30,8 +30,9 @@ struct PrefillKCfg {
     // q_full[2] k_full/k_empty/v_full/v_empty[NS] s_full[2] p_full[2][2] m_full[2][4] o_ready[2] o_done[2]
     static constexpr int N_BARS = 2 + 4 * P::NS + 2 + 4 + 8 + 2 + 2;
     // + mstat[2 tiles][2 block parities][128 rows] float2 + lsum[2 tiles][2 halves][128 rows] float
+    // + lscale[2 tiles][128 rows] float
     static constexpr int SMEM_BYTES = (2 + 2 * P::NS) * P::TILE + 1024 /*align*/ + N_BARS * 8 + 16 + 2 * 2 * 128 * 8 +
-                                      2 * 2 * 128 * 4;
+                                      2 * 2 * 128 * 4 + 2 * 128 * 4;
     static constexpr int REG_EXP = 128, REG_MAX = 80, REG_MISC = 56;   // 256 (128 + 80) + 128 * 56 <= 640 * 96
 };
 
@@ -59,7 +60,7 @@ struct RowStat {
 template <int EB, bool FOLD>
 __device__ __forceinline__ void prefill_max_warp(const FwdParams& p, int t, int wq, int lane, uint32_t tbase,
                                                  uint64_t* s_full_t, uint64_t* m_full_w, RowStat* mstat_t,
-                                                 uint64_t* o_ready_t, int n_t, int row0, int bh, int kvh) {
+                                                 float* lscale_t, uint64_t* o_ready_t, int n_t, int row0, int bh, int kvh) {
     using C = PrefillCfg<EB>;
     const uint32_t tlane = tbase + (static_cast<uint32_t>(wq * 32) << 16);
     const uint32_t tS = tlane + C::TM_S + t * 128, tO = tlane + C::TM_O + t * 128;
@@ -69,8 +70,10 @@ __device__ __forceinline__ void prefill_max_warp(const FwdParams& p, int t, int 
     float c_nat = p.sm_scale;
     if constexpr (EB == 1) c_nat *= p.q_scale[bh] * p.k_scale[kvh];
     const float cl2 = c_nat * LOG2E;
-    const float log2S = FOLD ? log2f(p.S) : 0.0f;   // exact for S = 2^k
+    const bool dynamic = p.scale_mode == 1;         // reading R26 (the host launches the FOLD instance for it)
+    const float log2S = (FOLD && !dynamic) ? log2f(p.S) : 0.0f;   // exact for S = 2^k
     float m_run = -INFINITY;
+    int k_run = 0;            // dynamic: the exponent O and the row sums carry
 
 #pragma unroll 1
     for (int c = 0; c < n_t; ++c) {
@@ -99,11 +102,21 @@ __device__ __forceinline__ void prefill_max_warp(const FwdParams& p, int t, int 
             }
         }
         // ---- lines 5-6 ----
-        const float m_new = fmaxf(m_run, fmaxf(m0, m1));
+        const float m_loc = fmaxf(m0, m1);
+        const float m_new = fmaxf(m_run, m_loc);
         const float m_used = (m_new == -INFINITY) ? 0.0f : m_new;
-        const float alpha = ptx::ex2_approx((m_run - m_used) * cl2);       // 0 when m_run = -inf
-        const float negm = fmaf(-m_used, cl2, log2S);
+        float alpha = ptx::ex2_approx((m_run - m_used) * cl2);             // 0 when m_run = -inf
+        float negm = fmaf(-m_used, cl2, log2S);
         m_run = m_new;
+        if (dynamic) {
+            // this block's scale 2^k goes into the exponent of P; what O and the row sums carry (the previous
+            // block's scale) is brought to it together with alpha -- exact, a power of two (Prop. 5)
+            const int k_new = (m_loc == -INFINITY) ? k_run : dyn_exponent((m_new - m_loc) * cl2);
+            negm = fmaf(-m_used, cl2, (float)k_new);
+            alpha *= exp2f((float)(k_new - k_run));
+            k_run = k_new;
+        }
+        if (c == n_t - 1) lscale_t[rl] = dynamic ? exp2f((float)k_run) : (FOLD ? p.S : 1.0f);   // read after o_done
         ptx::st_shared_v2(mstat_t + (c & 1) * 128 + rl, negm, alpha);
         __syncwarp();
         if (lane == 0) ptx::mbar_arrive(m_full_w);
@@ -144,11 +157,11 @@ __device__ __forceinline__ void prefill_max_warp(const FwdParams& p, int t, int 
 template <int EB, bool FOLD, int NPOLY, bool AUX>
 __device__ __forceinline__ void p_quarter(const uint32_t* v, uint32_t tS, int quarter, int j0, int jlim, uint64_t cl2_2,
                                           uint64_t negm_2, uint64_t s_2, uint64_t& sum_a, uint64_t& sum_b, uint64_t* bar,
-                                          int lane, uint8_t* dump_row, uint32_t* uf, int n_sink) {
+                                          int lane, uint8_t* dump_row, uint32_t* uf, const FwdParams& p) {
     using C = PrefillCfg<EB>;
     uint32_t w[C::P_COLS / 4];
     exp_chunk<EB, FOLD, false, NPOLY>(v, w, j0 + quarter * 32, jlim, cl2_2, negm_2, s_2, sum_a, sum_b);
-    if constexpr (AUX) chunk_statistics<EB>(w, j0 + quarter * 32, jlim, dump_row, uf, n_sink);
+    if constexpr (AUX) chunk_statistics<EB>(w, j0 + quarter * 32, jlim, dump_row, uf, p);
     if constexpr (EB == 1) ptx::tmem_st_x8(tS + quarter * 32, w);
     else ptx::tmem_st_x16(tS + quarter * 32, w);
     ptx::tmem_wait_st();
@@ -161,6 +174,7 @@ __device__ __forceinline__ void p_quarter(const uint32_t* v, uint32_t tS, int qu
 template <int EB, bool FOLD, bool AUX>
 __device__ __forceinline__ void prefill_exp_warp(const FwdParams& p, int wq, int half, int lane, uint32_t tbase,
                                                  uint64_t* m_full, uint64_t* p_full, const RowStat* mstat, float* lsum,
+                                                 const float* lscale,
                                                  uint64_t* o_done, const int* n_tile, int n_it, int pair, int bh,
                                                  int kvh, const CUtensorMap* mapO, uint8_t* stage0, uint8_t* stage1) {
     using C = PrefillCfg<EB>;
@@ -234,16 +248,16 @@ __device__ __forceinline__ void prefill_exp_warp(const FwdParams& p, int wq, int
             // AUX: the counter this block adds to (blocks that hold a sink key / all others); rows >= Lq do not
             // exist and are not counted
             uint32_t* const uf = (AUX && p.underflow != nullptr && (pair * 2 + t) * BM + rl < p.Lq)
-                                     ? (j0 < p.n_sink ? &uf_sink : &uf_other)
+                                     ? (sink_in_range(p, j0, 128) ? &uf_sink : &uf_other)
                                      : nullptr;
             p_quarter<EB, FOLD, CK::NPOLY, AUX>(r, tS, 2 * half, j0, jlim[t], cl2_2, negm_2, s_2, sum_a, sum_b,
-                                                p_full + 2 * t + 0, lane, dump_row[t], uf, p.n_sink);
+                                                p_full + 2 * t + 0, lane, dump_row[t], uf, p);
             if (probe_next) {
                 ptx::mbar_probe(m_full + 4 * (t ^ 1) + wq, c_o & 1);
                 probed_tile = t ^ 1;
             }
             p_quarter<EB, FOLD, CK::NPOLY, AUX>(r + 32, tS, 2 * half + 1, j0, jlim[t], cl2_2, negm_2, s_2, sum_a,
-                                                sum_b, p_full + 2 * t + 1, lane, dump_row[t], uf, p.n_sink);
+                                                sum_b, p_full + 2 * t + 1, lane, dump_row[t], uf, p);
             float sa, sb, sc, sd;
             ptx::unpack2(sum_a, sa, sb);
             ptx::unpack2(sum_b, sc, sd);
@@ -278,8 +292,10 @@ __device__ __forceinline__ void prefill_exp_warp(const FwdParams& p, int wq, int
         const int row0 = (pair * 2 + t) * BM;
         const int qrow = row0 + rl;
         const float l_all = lsum[(t * 2) * 128 + rl] + lsum[(t * 2 + 1) * 128 + rl];
-        if (qrow < p.Lq && half == 0 && p.row_sum != nullptr)
-            p.row_sum[(long long)bh * p.Lq + qrow] = FOLD ? l_all / p.S : l_all;
+        // l_all and O carry the same factor: S when the static scale is folded into the exponent, the last
+        // block's 2^k under the dynamic scale (published by the max warp), 1 otherwise
+        const float carried = (n_tile[t] > 0) ? lscale[t * 128 + rl] : 1.0f;
+        if (qrow < p.Lq && half == 0 && p.row_sum != nullptr) p.row_sum[(long long)bh * p.Lq + qrow] = l_all / carried;
         const float inv = (l_all > 0.0f) ? (FOLD ? vs / l_all : vs / (p.S * l_all)) : 0.0f;
         if (row0 >= p.Lq) continue;             // no row of this tile exists (warp-uniform)
         const uint32_t tO = tlane + C::TM_O + t * 128 + half * 64;
@@ -294,6 +310,25 @@ __device__ __forceinline__ void prefill_exp_warp(const FwdParams& p, int wq, int
             } else {
 #pragma unroll
                 for (int e = 0; e < 32; ++e) v[e] = 0u;
+            }
+            if (p.o_bf16) {
+                // one 32-row x 64-column BF16 box (128-byte rows) per warp and tile: chunk cb fills half of it
+                uint8_t* box = stage + (half * 8 + wq) * 4096;
+#pragma unroll
+                for (int j = 0; j < 4; ++j) {
+                    uint4 w4;
+                    w4.x = ptx::cvt_bf16x2(__uint_as_float(v[8 * j]) * inv, __uint_as_float(v[8 * j + 1]) * inv);
+                    w4.y = ptx::cvt_bf16x2(__uint_as_float(v[8 * j + 2]) * inv, __uint_as_float(v[8 * j + 3]) * inv);
+                    w4.z = ptx::cvt_bf16x2(__uint_as_float(v[8 * j + 4]) * inv, __uint_as_float(v[8 * j + 5]) * inv);
+                    w4.w = ptx::cvt_bf16x2(__uint_as_float(v[8 * j + 6]) * inv, __uint_as_float(v[8 * j + 7]) * inv);
+                    *reinterpret_cast<uint4*>(box + lane * 128 + (((cb * 4 + j) ^ (lane & 7)) << 4)) = w4;
+                }
+                if (cb == 1) {
+                    ptx::fence_proxy_async_smem();
+                    __syncwarp();
+                    if (lane == 0) ptx::tma_store_3d(mapO, box, half * 64, row0 + wq * 32, bh);
+                }
+                continue;
             }
             uint8_t* box = stage + (ch * 4 + wq) * 4096;
 #pragma unroll
@@ -340,6 +375,7 @@ attn_prefill_kernel(const __grid_constant__ CUtensorMap mapQ, const __grid_const
     uint32_t* tmem_slot = reinterpret_cast<uint32_t*>(o_done + 2);
     RowStat* mstat = reinterpret_cast<RowStat*>(tmem_slot + 4);   // [2 tiles][2 block parities][128 rows]
     float* lsum = reinterpret_cast<float*>(mstat + 2 * 2 * 128);  // [2 tiles][2 halves][128 rows]
+    float* lscale = lsum + 2 * 2 * 128;                           // [2 tiles][128 rows]  factor the row sums carry
 
     const int tid = threadIdx.x, lane = tid & 31;
     const int warp = __shfl_sync(0xFFFFFFFFu, tid >> 5, 0);   // provably warp-uniform
@@ -406,13 +442,13 @@ attn_prefill_kernel(const __grid_constant__ CUtensorMap mapQ, const __grid_const
 
     if (warp < 8) {
         ptx::setmaxnreg_inc<C4::REG_EXP>();
-        prefill_exp_warp<EB, FOLD, AUX>(p, warp & 3, warp >> 2, lane, tbase, m_full, p_full, mstat, lsum, o_done, n_tile,
+        prefill_exp_warp<EB, FOLD, AUX>(p, warp & 3, warp >> 2, lane, tbase, m_full, p_full, mstat, lsum, lscale, o_done, n_tile,
                                         n_it, pair, bh, kvh, &mapO, sK, sV);
     } else if (warp < 16) {
         ptx::setmaxnreg_dec<C4::REG_MAX>();
         const int t = (warp - 8) >> 2, wq = warp & 3;
         prefill_max_warp<EB, FOLD>(p, t, wq, lane, tbase, s_full + t, m_full + 4 * t + wq, mstat + t * 2 * 128,
-                                   o_ready + t, n_tile[t], (pair * 2 + t) * BM, bh, kvh);
+                                   lscale + t * 128, o_ready + t, n_tile[t], (pair * 2 + t) * BM, bh, kvh);
     } else {
         ptx::setmaxnreg_dec<C4::REG_MISC>();
         if (warp == 18) {

@@ -140,7 +140,7 @@ __device__ __forceinline__ void prefill64_softmax(const FwdParams& p, int t, int
             else exp_chunk<EB, FOLD, false>(v, w, j0 + cb * 32, jlim, cl2_2, negm_2, s_2, sum_a, sum_b);
             if constexpr (AUX)
                 chunk_statistics<EB>(w, j0 + cb * 32, jlim, dump_row,
-                                     count ? (j0 < p.n_sink ? &uf_sink : &uf_other) : nullptr, p.n_sink);
+                                     count ? (sink_in_range(p, j0, C::BN) ? &uf_sink : &uf_other) : nullptr, p);
             // (P of chunk cb lands on columns of chunk 0, whose logits are already in registers)
             if constexpr (EB == 1) ptx::tmem_st_x8(tS + cb * 8, w);
             else ptx::tmem_st_x16(tS + cb * 16, w);
@@ -204,7 +204,7 @@ __device__ __forceinline__ void prefill64_softmax(const FwdParams& p, int t, int
         ptx::mbar_wait(o_done, 0);
         ptx::tc_fence_after();
     }
-    float* dst = p.o + grow * C::D + par * 64;     // this warp stores columns 64 par .. 64 par + 63
+    const long long dst = grow * C::D + par * 64;  // this warp stores columns 64 par .. 64 par + 63
 #pragma unroll 1
     for (int cb = 0; cb < 2; ++cb) {
         uint32_t v[32];
@@ -221,7 +221,7 @@ __device__ __forceinline__ void prefill64_softmax(const FwdParams& p, int t, int
                 float4 o4 = make_float4(__uint_as_float(v[e]) * inv, __uint_as_float(v[e + 1]) * inv,
                                         __uint_as_float(v[e + 2]) * inv, __uint_as_float(v[e + 3]) * inv);
                 if (l_all <= 0.0f) o4 = make_float4(0.f, 0.f, 0.f, 0.f);
-                *reinterpret_cast<float4*>(dst + cb * 32 + e) = o4;
+                store_o4(p, dst + cb * 32 + e, o4.x, o4.y, o4.z, o4.w);
             }
         }
     }

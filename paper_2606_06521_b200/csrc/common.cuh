@@ -8,8 +8,12 @@ namespace fp8attn {
 constexpr int BM = 128;   // query rows per tile = UMMA M = TMEM lanes
 constexpr float LOG2E = 1.4426950408889634f;
 
+constexpr int MAX_SINKS = 32;          // FP8ATTN_MAX_SINKS
+constexpr int DYN_K_MAX = 30;          // largest exponent of the dynamic P scale (reading R26)
+constexpr float LOG2_448 = 8.80735492205760410744f;
+
 struct FwdParams {
-    float* o;
+    void* o;          // float32, or bfloat16 when o_bf16
     float* row_max;
     float* row_sum;
     unsigned long long* underflow;
@@ -23,6 +27,48 @@ struct FwdParams {
     int B, Hq, Hkv, Lq, Lk, causal, kv_order, n_sink, num_splits, nb;
     int q_slabs, kv_slabs;   // B*Hq, B*Hkv: plane stride of the staged operands, in slabs
     float S, sm_scale;
+    int scale_mode;          // 1: dynamic per-(row, block) power-of-two scale
+    int o_bf16;
+    int n_sinkpos;           // -1: the sink keys are the first n_sink keys; else sink_pos[0 .. n_sinkpos) (ascending)
+    int sink_pos[MAX_SINKS];
 };
+
+// ---- sink keys (underflow classification, Prop. 1 / PAPER.md:443) and the block order (Alg. 1 line 2) ----
+__device__ __forceinline__ bool sink_in_range(const FwdParams& p, int j0, int n) {     // a sink key in [j0, j0 + n)?
+    if (p.n_sinkpos < 0) return j0 < p.n_sink;
+    bool any = false;
+    for (int s = 0; s < p.n_sinkpos; ++s) any |= (p.sink_pos[s] >= j0 && p.sink_pos[s] < j0 + n);
+    return any;
+}
+__device__ __forceinline__ bool is_sink_key(const FwdParams& p, int j) { return sink_in_range(p, j, 1); }
+// Block visited at step `step` of the block range [b0, b1): forward, reverse, or sink blocks last (the blocks
+// without a sink key in descending order, then those with one, in descending order; reading R27).
+__device__ __forceinline__ int block_at(const FwdParams& p, int b0, int b1, int step, int bn) {
+    if (p.kv_order == 0) return b0 + step;
+    if (p.kv_order == 1) return b1 - 1 - step;
+    int seen = 0;
+    for (int pass = 0; pass < 2; ++pass)
+        for (int b = b1 - 1; b >= b0; --b)
+            if ((int)sink_in_range(p, b * bn, bn) == pass) {
+                if (seen == step) return b;
+                ++seen;
+            }
+    return b0;
+}
+// Exponent of the dynamic scale of a block: the largest k <= DYN_K_MAX with 2^k * 2^(-g2) <= 448, where
+// g2 = (m_new - m_loc) in base-2 units of the scaled logit (>= 0); both in FP32 (reading R26).
+__device__ __forceinline__ int dyn_exponent(float g2) {
+    const int k = (int)floorf(g2 + LOG2_448);
+    return k > DYN_K_MAX ? DYN_K_MAX : k;
+}
+// o element stores
+__device__ __forceinline__ void store_o4(const FwdParams& p, long long idx, float a, float b, float c, float d) {
+    if (p.o_bf16) {
+        uint2 w = make_uint2(ptx::cvt_bf16x2(a, b), ptx::cvt_bf16x2(c, d));
+        *reinterpret_cast<uint2*>(static_cast<uint16_t*>(p.o) + idx) = w;
+    } else {
+        *reinterpret_cast<float4*>(static_cast<float*>(p.o) + idx) = make_float4(a, b, c, d);
+    }
+}
 
 }  // namespace fp8attn

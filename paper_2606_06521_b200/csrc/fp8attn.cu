@@ -224,9 +224,9 @@ int launch_prefill(const CUtensorMap& mq, const CUtensorMap& mk, const CUtensorM
     // the statistics instance (P dump, underflow counters of fp8attn_stats) has the same schedule; the plain
     // instance carries none of that code
     const bool aux = p.p_codes || p.underflow;
-    // o as [B*Hq, Lq, d] FP32: boxes of 32 rows x 32 floats, stored by TMA from the epilogue
+    // o as [B*Hq, Lq, d]: boxes of 32 rows x 128 bytes (32 floats / 64 bfloat16), stored by TMA from the epilogue
     CUtensorMap mo;
-    if (int rc = make_map(&mo, p.o, 4, (long long)p.B * p.Hq, p.Lq, 128, 32)) return rc;
+    if (int rc = make_map(&mo, p.o, p.o_bf16 ? 2 : 4, (long long)p.B * p.Hq, p.Lq, 128, 32)) return rc;
     const dim3 grid((unsigned)(((p.Lq + 2 * BM - 1) / (2 * BM)) * (p.B * p.Hq)));
     if (aux) {
         auto kern = attn_prefill_kernel<EB, FOLD, true>;
@@ -320,7 +320,7 @@ int validate_args(const void* q, const void* k, const void* v, const void* o, in
     if (!(S > 0.0f) || !std::isfinite(S)) return FP8ATTN_E_SCALE;
     const int pm = mode & 0xFF, dt = (mode >> 8) & 0xF;
     if ((mode & ~0xFFF) || pm > 2 || dt > 3) return FP8ATTN_E_MODE;
-    if (kv_order != FP8ATTN_ORDER_FORWARD && kv_order != FP8ATTN_ORDER_REVERSE) return FP8ATTN_E_MODE;
+    if (kv_order < FP8ATTN_ORDER_FORWARD || kv_order > FP8ATTN_ORDER_SINK_LAST) return FP8ATTN_E_MODE;
     const bool e4m3_kv = (dt == 2 || dt == 3);
     if ((pm == FP8ATTN_MODE_FP8) != e4m3_kv) return FP8ATTN_E_MODE;
     if (stats && stats->struct_size != (int32_t)sizeof(fp8attn_stats)) return FP8ATTN_E_STATS;
@@ -334,7 +334,16 @@ int validate_args(const void* q, const void* k, const void* v, const void* o, in
     if (dt == 0 && bn == 128) return FP8ATTN_E_UNSUPPORTED;
     const int ns = stats ? stats->num_splits : 0;
     if (ns < 0 || ns > FP8ATTN_MAX_SPLITS) return FP8ATTN_E_UNSUPPORTED;
-    if (stats && (stats->kernel < 0 || stats->kernel > 3 || stats->reserved0 != 0)) return FP8ATTN_E_MODE;
+    if (stats && (stats->kernel < 0 || stats->kernel > 3 || stats->reserved1 != 0)) return FP8ATTN_E_MODE;
+    if (stats && (stats->scale_mode < 0 || stats->scale_mode > 1 || stats->o_dtype < 0 || stats->o_dtype > 1)) return FP8ATTN_E_MODE;
+    if (stats && stats->scale_mode == FP8ATTN_SCALE_DYNAMIC && pm == FP8ATTN_MODE_NOCAST) return FP8ATTN_E_MODE;
+    if (stats && stats->n_sink < 0) return FP8ATTN_E_SHAPE;
+    if (stats && stats->sink_pos) {
+        if (stats->n_sink < 1 || stats->n_sink > FP8ATTN_MAX_SINKS) return FP8ATTN_E_SHAPE;
+        for (int i = 0; i < stats->n_sink; ++i)
+            if (stats->sink_pos[i] < 0 || stats->sink_pos[i] >= Lk || (i > 0 && stats->sink_pos[i] <= stats->sink_pos[i - 1]))
+                return FP8ATTN_E_SHAPE;
+    }
     if (stats && stats->p_codes && (stats->p_batch < 0 || stats->p_batch >= B || stats->p_head < 0 || stats->p_head >= Hq))
         return FP8ATTN_E_SHAPE;
     if ((long long)B * Hq * ((Lq + 127) / 128) > 0x7FFFFFFFll) return FP8ATTN_E_UNSUPPORTED;
@@ -469,7 +478,7 @@ int fp8attn_fwd(const void* q, const void* k, const void* v, void* o, int B, int
 
     FwdParams p;
     memset(&p, 0, sizeof p);
-    p.o = static_cast<float*>(o);
+    p.o = o;
     p.row_max = stats ? stats->row_max : nullptr;
     p.row_sum = stats ? stats->row_sum : nullptr;
     p.underflow = stats ? stats->underflow : nullptr;
@@ -482,6 +491,14 @@ int fp8attn_fwd(const void* q, const void* k, const void* v, void* o, int B, int
     p.causal = causal ? 1 : 0;
     p.kv_order = kv_order;
     p.n_sink = stats ? stats->n_sink : 0;
+    p.scale_mode = stats ? stats->scale_mode : 0;
+    p.o_bf16 = (stats && stats->o_dtype == FP8ATTN_O_BF16) ? 1 : 0;
+    p.n_sinkpos = -1;
+    if (stats && stats->sink_pos) {
+        p.n_sinkpos = stats->n_sink;
+        for (int i = 0; i < stats->n_sink; ++i) p.sink_pos[i] = stats->sink_pos[i];
+    }
+    const bool dynamic = p.scale_mode == 1;
     p.num_splits = ns;
     p.nb = nb;
     p.q_slabs = (int)q_slabs;
@@ -503,7 +520,9 @@ int fp8attn_fwd(const void* q, const void* k, const void* v, void* o, int B, int
     // modes 1 and 2 (Bn = 128 and Bn = 64); the decode kernel serves decode shapes with any split count; each
     // has a statistics instance (same schedule + P dump + underflow counters).  Everything else -- FP32
     // inputs, the no-cast mode, d = 64, prefill with splits -- runs on the general kernel.
-    const bool prefill_ok = d == 128 && ns == 1 && npl == 1 && pm != 0 && dt != 3;
+    // (not built into the prefill kernels: the sink-blocks-last order; the dynamic scale with Bn = 64)
+    const bool prefill_ok = d == 128 && ns == 1 && npl == 1 && pm != 0 && dt != 3 && kv_order != FP8ATTN_ORDER_SINK_LAST &&
+                            !(dynamic && bn == 64);
     if (want_kernel == 2 && !prefill_ok) return FP8ATTN_E_UNSUPPORTED;
     // (automatic selection keeps prefill-shaped calls that ask for the P dump or the underflow counters on the
     // general kernel, whose serial schedule is the reference for them; stats->kernel = 2 takes the statistics
@@ -517,10 +536,11 @@ int fp8attn_fwd(const void* q, const void* k, const void* v, void* o, int B, int
         CUtensorMap mq16;
         if (int rc2 = make_map(&mq16, qs, 1, 1, q_slabs * Lq, d, 16)) return rc2;
         const int nv = (Hq / Hkv) * Lq;
-        rc = is_pow2_scale(S) ? launch_decode<true>(nv, mq16, mk, mv, p, st) : launch_decode<false>(nv, mq16, mk, mv, p, st);
+        rc = (is_pow2_scale(S) || dynamic) ? launch_decode<true>(nv, mq16, mk, mv, p, st)
+                                           : launch_decode<false>(nv, mq16, mk, mv, p, st);
     } else if (use_prefill) {
         kernel_id = 2;
-        const bool fold = is_pow2_scale(S);
+        const bool fold = is_pow2_scale(S) || dynamic;      // the dynamic 2^k goes through the folded-scale instance
         if (bn == 64) {
             if (eb == 1) rc = fold ? launch_prefill64<1, true>(mq, mk, mv, p, st) : launch_prefill64<1, false>(mq, mk, mv, p, st);
             else rc = fold ? launch_prefill64<2, true>(mq, mk, mv, p, st) : launch_prefill64<2, false>(mq, mk, mv, p, st);
@@ -543,7 +563,7 @@ int fp8attn_fwd(const void* q, const void* k, const void* v, void* o, int B, int
         const int rows_per_block = 8;
         combine_kernel<<<(unsigned)((R + rows_per_block - 1) / rows_per_block), rows_per_block * 32, 0, st>>>(
             p.part_o, p.part_ml, p.o, p.row_max, p.row_sum, (pm == 2) ? p.v_scale : nullptr, R, d, ns,
-            (pm == 0) ? 1.0f : S, Hq, Hkv, Lq);
+            (pm == 0 || dynamic) ? 1.0f : S, Hq, Hkv, Lq, p.o_bf16);
         CU_TRY(cudaGetLastError());
         ++n_launches;
     }
@@ -574,7 +594,8 @@ int fp8attn_fwd_host(const void* q, const void* k, const void* v, void* o, int B
     const size_t o_q = off;   off += up(nq * ebq);
     const size_t o_k = off;   off += up(nkv * ebkv);
     const size_t o_v = off;   off += up(nkv * ebkv);
-    const size_t o_o = off;   off += up(nq * 4);
+    const size_t ebo = (stats && stats->o_dtype == FP8ATTN_O_BF16) ? 2 : 4;
+    const size_t o_o = off;   off += up(nq * ebo);
     const size_t o_qs = off;  off += up(nqs * 4);
     const size_t o_ks = off;  off += up(nkvs * 4);
     const size_t o_vs = off;  off += up(nkvs * 4);
@@ -630,7 +651,7 @@ int fp8attn_fwd_host(const void* q, const void* k, const void* v, void* o, int B
     // of piece i-1 overlap on three streams (PCIe is full duplex).  The P dump and the underflow counters belong
     // to one whole call and keep the single-piece path.
     int pieces_b = 1, pieces_h = 1;      // pieces along the batch, and along the kv heads of one batch element
-    const size_t traffic = nq * ebq + 2 * nkv * ebkv + nq * 4;
+    const size_t traffic = nq * ebq + 2 * nkv * ebkv + nq * ebo;
     // (the automatic split count of a decode-shaped call depends on B * Hkv: such a call stays whole unless the
     // caller fixes num_splits, otherwise the pieces would take another split layout than the single call, R14)
     const bool auto_split = (long long)(Hq / Hkv) * Lq <= 16 && !(stats && stats->num_splits > 0);
@@ -648,7 +669,7 @@ int fp8attn_fwd_host(const void* q, const void* k, const void* v, void* o, int B
         if (int rc = fp8attn_fwd(base + o_q, base + o_k, base + o_v, base + o_o, B, Hq, Hkv, Lq, Lk, d, causal, S,
                                  kv_order, mode, ds))
             return rc;
-        CU_TRY(cudaMemcpyAsync(o, base + o_o, nq * 4, cudaMemcpyDeviceToHost, st));
+        CU_TRY(cudaMemcpyAsync(o, base + o_o, nq * ebo, cudaMemcpyDeviceToHost, st));
         if (stats) {
             if (stats->row_max) CU_TRY(cudaMemcpyAsync(stats->row_max, base + o_rm, R * 4, cudaMemcpyDeviceToHost, st));
             if (stats->row_sum) CU_TRY(cudaMemcpyAsync(stats->row_sum, base + o_rs, R * 4, cudaMemcpyDeviceToHost, st));
@@ -704,7 +725,7 @@ int fp8attn_fwd_host(const void* q, const void* k, const void* v, void* o, int B
                 if (ps.row_sum) ps.row_sum += q_slab0 * Lq;
             }
             if (int rc = fp8attn_fwd(base + o_q + q_el * ebq, base + o_k + kv_el * ebkv, base + o_v + kv_el * ebkv,
-                                     base + o_o + q_el * 4, b1 - b0, pieces_h > 1 ? hq_p : Hq, pieces_h > 1 ? hkv_p : Hkv,
+                                     base + o_o + q_el * ebo, b1 - b0, pieces_h > 1 ? hq_p : Hq, pieces_h > 1 ? hkv_p : Hkv,
                                      Lq, Lk, d, causal, S, kv_order, mode, pp))
                 return rc;
             if (pp) {
@@ -718,7 +739,7 @@ int fp8attn_fwd_host(const void* q, const void* k, const void* v, void* o, int B
             }
             CU_TRY(cudaEventRecord(ev_done[i], st));
             CU_TRY(cudaStreamWaitEvent(s_out, ev_done[i], 0));
-            CU_TRY(cudaMemcpyAsync(ho + q_el * 4, base + o_o + q_el * 4, q_n * 4, cudaMemcpyDeviceToHost, s_out));
+            CU_TRY(cudaMemcpyAsync(ho + q_el * ebo, base + o_o + q_el * ebo, q_n * ebo, cudaMemcpyDeviceToHost, s_out));
             if (stats && stats->row_max)
                 CU_TRY(cudaMemcpyAsync(stats->row_max + q_slab0 * Lq, base + o_rm + q_slab0 * Lq * 4,
                                        (size_t)(b1 - b0) * hq_p * Lq * 4, cudaMemcpyDeviceToHost, s_out));

@@ -132,10 +132,11 @@ __device__ __forceinline__ void mask32(uint32_t* v, int j_first, int jlim) {
 // exp_chunk leaves it; BF16 mode recovers a code from its exact BF16 value: times 2^-120, shifted right by 4.
 template <int EB>
 __device__ __forceinline__ void chunk_statistics(const uint32_t* w, int jq, int jlim, uint8_t* dump_row, uint32_t* uf,
-                                                 int n_sink) {
+                                                 const FwdParams& p) {
     constexpr int NW = 8 * EB;      // words of the chunk
     if (dump_row == nullptr && uf == nullptr) return;
-    if (dump_row == nullptr && jq >= n_sink && jq + 31 <= jlim) {
+    const bool has_sink = sink_in_range(p, jq, 32);
+    if (dump_row == nullptr && !has_sink && jq + 31 <= jlim) {
         // every key of the chunk is visible and none is a sink: count the zero codes a word at a time
         uint32_t zeros = 0;
 #pragma unroll
@@ -157,7 +158,7 @@ __device__ __forceinline__ void chunk_statistics(const uint32_t* w, int jq, int 
         }
         const bool vis = jq + e <= jlim;
         if (vis && dump_row != nullptr) dump_row[jq + e] = (uint8_t)code;
-        if (vis && jq + e >= n_sink && code == 0) ++zeros;
+        if (vis && code == 0 && !(has_sink && is_sink_key(p, jq + e))) ++zeros;
     }
     if (uf != nullptr) *uf += zeros;
 }

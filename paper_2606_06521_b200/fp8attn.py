@@ -18,7 +18,8 @@ from .build import LIB, build
 
 MODE_NOCAST, MODE_ISOLATION, MODE_FP8 = 0, 1, 2
 DTYPE_F32, DTYPE_BF16, DTYPE_E4M3, DTYPE_BF16Q_E4M3KV = 0 << 8, 1 << 8, 2 << 8, 3 << 8
-ORDER_FORWARD, ORDER_REVERSE = 0, 1
+ORDER_FORWARD, ORDER_REVERSE, ORDER_SINK_LAST = 0, 1, 2
+SCALE_STATIC, SCALE_DYNAMIC = 0, 1
 MAX_SPLITS = 64
 
 
@@ -26,10 +27,11 @@ class Stats(C.Structure):
     """struct fp8attn_stats"""
     _fields_ = [
         ("struct_size", C.c_int32), ("n_sink", C.c_int32), ("block_n", C.c_int32),
-        ("num_splits", C.c_int32), ("kernel", C.c_int32), ("reserved0", C.c_int32),
+        ("num_splits", C.c_int32), ("kernel", C.c_int32), ("scale_mode", C.c_int32),
         ("q_scale", C.c_void_p), ("k_scale", C.c_void_p), ("v_scale", C.c_void_p),
         ("stream", C.c_void_p), ("p_codes", C.c_void_p),
         ("p_batch", C.c_int32), ("p_head", C.c_int32),
+        ("sink_pos", C.c_void_p), ("o_dtype", C.c_int32), ("reserved1", C.c_int32),
         ("row_max", C.c_void_p), ("row_sum", C.c_void_p), ("underflow", C.c_void_p),
         ("block_m_used", C.c_int32), ("block_n_used", C.c_int32), ("num_splits_used", C.c_int32),
         ("split_bounds", C.c_int32 * (MAX_SPLITS + 1)),
@@ -100,6 +102,16 @@ def _ptr(t: Optional[torch.Tensor]):
     return None if t is None else C.c_void_p(t.data_ptr())
 
 
+def _set_sinks(st, sink_pos, keep):
+    """sink_pos (host list of ascending key indices) -> st.sink_pos / st.n_sink."""
+    if sink_pos is None:
+        return
+    arr = (C.c_int32 * len(sink_pos))(*[int(x) for x in sink_pos])
+    keep.append(arr)
+    st.sink_pos = C.cast(arr, C.c_void_p)
+    st.n_sink = len(sink_pos)
+
+
 @dataclass
 class FwdResult:
     o: torch.Tensor                       # [B,Hq,Lq,d] float32
@@ -131,11 +143,12 @@ def _dtype_code(q, k):
 def fwd(q, k, v, *, causal: bool, S: float, kv_order: int, mode: int, n_sink: int = 4,
         block_n: int = 0, num_splits: int = 0, kernel: int = 0, q_scale=None, k_scale=None, v_scale=None,
         want_stats: bool = False, want_underflow: Optional[bool] = None, dump_head=None, out=None,
-        stream=None) -> FwdResult:
+        stream=None, scale_mode: int = 0, sink_pos=None, out_dtype=None) -> FwdResult:
     """fp8attn_fwd on CUDA tensors q [B,Hq,Lq,d], k/v [B,Hkv,Lk,d] (contiguous).  `mode` is the
     P mode (0 no-cast, 1 isolation, 2 FP8); the input dtype bits are derived from the tensors.
     `dump_head=(b,h)` returns the E4M3 code of every P of that head.  `kernel` requests a kernel
-    family (0 automatic, 1 general, 2 prefill, 3 decode)."""
+    family (0 automatic, 1 general, 2 prefill, 3 decode).  `scale_mode=1`: dynamic per-(row, block) 2^k scale;
+    `sink_pos`: ascending key indices of the sink keys (replaces n_sink); `out_dtype=torch.bfloat16`: BF16 output."""
     for t in (q, k, v):
         if not (t.is_cuda and t.is_contiguous() and t.dim() == 4):
             raise ValueError("q, k, v must be contiguous 4-D CUDA tensors")
@@ -143,12 +156,20 @@ def fwd(q, k, v, *, causal: bool, S: float, kv_order: int, mode: int, n_sink: in
     Bk, Hkv, Lk, dk = k.shape
     if (Bk, dk) != (B, d) or v.shape != k.shape:
         raise ValueError("shape mismatch between q, k, v")
-    o = out if out is not None else torch.empty((B, Hq, Lq, d), dtype=torch.float32, device=q.device)
+    if out is not None:
+        out_dtype = out.dtype
+    out_dtype = torch.float32 if out_dtype is None else out_dtype
+    if out_dtype not in (torch.float32, torch.bfloat16):
+        raise TypeError("o must be float32 or bfloat16")
+    o = out if out is not None else torch.empty((B, Hq, Lq, d), dtype=out_dtype, device=q.device)
     st = Stats()
     st.struct_size = C.sizeof(Stats)
     st.n_sink, st.block_n, st.num_splits, st.kernel = n_sink, block_n, num_splits, kernel
+    st.scale_mode = int(scale_mode)
+    st.o_dtype = 1 if out_dtype == torch.bfloat16 else 0
     st.stream = _stream_ptr(stream)
     keep = []
+    _set_sinks(st, sink_pos, keep)
     for name, t in (("q_scale", q_scale), ("k_scale", k_scale), ("v_scale", v_scale)):
         if t is not None:
             t = t.to(device=q.device, dtype=torch.float32).contiguous()
@@ -178,7 +199,7 @@ def fwd(q, k, v, *, causal: bool, S: float, kv_order: int, mode: int, n_sink: in
 def fwd_host(q, k, v, *, causal: bool, S: float, kv_order: int, mode: int, n_sink: int = 4,
              block_n: int = 0, num_splits: int = 0, kernel: int = 0, q_scale=None, k_scale=None, v_scale=None,
              want_stats: bool = False, want_underflow: Optional[bool] = None, out=None, stream=None,
-             device=None) -> FwdResult:
+             device=None, scale_mode: int = 0, sink_pos=None, out_dtype=None) -> FwdResult:
     """fp8attn_fwd_host on HOST tensors (CPU, ideally pinned): the library copies them to the
     device, runs the kernels, copies `o` (and statistics) back and synchronises the stream."""
     for t in (q, k, v):
@@ -188,11 +209,17 @@ def fwd_host(q, k, v, *, causal: bool, S: float, kv_order: int, mode: int, n_sin
     Bk, Hkv, Lk, dk = k.shape
     if (Bk, dk) != (B, d) or v.shape != k.shape:
         raise ValueError("shape mismatch between q, k, v")
-    o = out if out is not None else torch.empty((B, Hq, Lq, d), dtype=torch.float32, pin_memory=True)
+    if out is not None:
+        out_dtype = out.dtype
+    out_dtype = torch.float32 if out_dtype is None else out_dtype
+    o = out if out is not None else torch.empty((B, Hq, Lq, d), dtype=out_dtype, pin_memory=True)
     st = Stats()
     st.struct_size = C.sizeof(Stats)
     st.n_sink, st.block_n, st.num_splits, st.kernel = n_sink, block_n, num_splits, kernel
+    st.scale_mode = int(scale_mode)
+    st.o_dtype = 1 if out_dtype == torch.bfloat16 else 0
     keep = []
+    _set_sinks(st, sink_pos, keep)
     for name, t in (("q_scale", q_scale), ("k_scale", k_scale), ("v_scale", v_scale)):
         if t is not None:
             t = t.to(device="cpu", dtype=torch.float32).contiguous()

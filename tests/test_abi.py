@@ -59,7 +59,7 @@ def test_argument_checks_precede_any_cuda_call(fa):
     assert f(one, one, one, one, 1, 1, 1, 1, 1, 64, 0, 0.0, 0, 1, None) == -3       # S
     assert f(one, one, one, one, 1, 1, 1, 1, 1, 64, 0, float("inf"), 0, 1, None) == -3
     assert f(one, one, one, one, 1, 1, 1, 1, 1, 64, 0, float("nan"), 0, 1, None) == -3
-    assert f(one, one, one, one, 1, 1, 1, 1, 1, 64, 0, 1.0, 2, 1, None) == -4       # kv_order
+    assert f(one, one, one, one, 1, 1, 1, 1, 1, 64, 0, 1.0, 3, 1, None) == -4       # kv_order (0, 1, 2 exist)
     assert f(one, one, one, one, 1, 1, 1, 1, 1, 64, 0, 1.0, 0, 3, None) == -4       # mode
     assert f(one, one, one, one, 1, 1, 1, 1, 1, 64, 0, 1.0, 0, 2, None) == -4       # FP8 mode, FP32 dtype
     assert f(one, one, one, one, 1, 1, 1, 1, 1, 128, 0, 1.0, 0, 2 | (2 << 8), None) == -1   # no scales
