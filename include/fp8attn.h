@@ -125,6 +125,22 @@ typedef struct fp8attn_stats {
                                   keys (multi-sink / distributed-sink layouts)    */
     int32_t o_dtype;           /* FP8ATTN_O_*                                                    */
     int32_t reserved1;         /* must be 0                                                      */
+    /* variable-length and paged KV-cache prefill / decode (the shape of the kernel the paper simulates,
+       attention_with_kvcache_prefill_fp8).  All optional.                              */
+    const int32_t *seqlens_q;  /* device [B] or NULL: batch element b has seqlens_q[b] <= Lq query rows
+                                  (q, o stay padded [B,Hq,Lq,d]); the rows beyond produce 0, like rows
+                                  that see no key.  The causal diagonal is bottom-right aligned per
+                                  batch element: key j visible to row i iff j <= i + seqlens_k[b] -
+                                  seqlens_q[b]                                                   */
+    const int32_t *seqlens_k;  /* device [B] or NULL: batch element b has seqlens_k[b] <= Lk keys    */
+    const int32_t *block_table;/* device [B, max_pages] or NULL.  Not NULL: k and v are page pools
+                                  [num_pages, Hkv, page_size, d]; key j of batch element b is row
+                                  j % page_size of page block_table[b][j / page_size].  page_size must
+                                  be a multiple of the KV block (block_n_used); BF16 / E4M3 k, v.
+                                  Memory of a page beyond the end of its sequence must hold finite
+                                  values (it is multiplied by P = 0)                             */
+    int32_t page_size, max_pages, num_pages;
+    int32_t reserved2;         /* must be 0                                                      */
     /* ---- outputs, device (each may be NULL) ---- */
     float *row_max;            /* [B,Hq,Lq] final running max m (scaled logits, natural log)    */
     float *row_sum;            /* [B,Hq,Lq] final l relative to m; NOT multiplied by S           */
@@ -146,7 +162,8 @@ typedef struct fp8attn_stats {
 /*
  * fp8attn_fwd -- attention forward (Alg. 1).
  *   q, o : device, [B, Hq, Lq, d] contiguous row-major; o is float32 (bfloat16 with stats->o_dtype).
- *   k, v : device, [B, Hkv, Lk, d]; query head h reads kv head h / (Hq / Hkv).
+ *   k, v : device, [B, Hkv, Lk, d] (or page pools, see stats->block_table; Lk is then the capacity
+ *          max_pages * page_size is checked against); query head h reads kv head h / (Hq / Hkv).
  *   d    : 64 or 128.  Softmax scale is 1/sqrt(d).
  *   causal : nonzero = key j visible to query i iff j <= i + (Lk - Lq) (bottom-right).
  *   S    : static P scale, finite > 0 (values above 448 saturate at 448).
@@ -172,6 +189,7 @@ FP8ATTN_API int fp8attn_fwd(const void *q, const void *k, const void *v, void *o
  *   and downloads overlap on `stats->stream` and two library-owned copy streams; the results are
  *   those of the single call bit for bit, `n_launches` counts every piece.
  * Every step of the method still runs in the CUDA kernels; the host side only copies.
+ * seqlens_q / seqlens_k / block_table are not taken here (FP8ATTN_E_UNSUPPORTED): a paged cache lives on the device.
  * Errors as fp8attn_fwd.
  */
 FP8ATTN_API int fp8attn_fwd_host(const void *q, const void *k, const void *v, void *o,

@@ -75,8 +75,9 @@ attn_decode_kernel(const __grid_constant__ CUtensorMap mapQ, const __grid_consta
     const int split = blockIdx.y;
     const int b = kvslab / p.Hkv, kvh_in_b = kvslab % p.Hkv;
     const long long row0 = ((long long)b * p.Hq + (long long)kvh_in_b * G) * p.Lq;   // first of the nv output rows
-    const int sb0 = (int)(((long long)split * p.nb) / p.num_splits);
-    const int sb1 = (int)(((long long)(split + 1) * p.nb) / p.num_splits);
+    const Seq sq = seq_of(p, b, DecodeCfg::BN);      // this batch element's lengths (variable-length sequences)
+    const int sb0 = (int)(((long long)split * sq.nb) / p.num_splits);
+    const int sb1 = (int)(((long long)(split + 1) * sq.nb) / p.num_splits);
     const int n_it = sb1 - sb0;
 
     if (tid == 0) {
@@ -121,12 +122,14 @@ attn_decode_kernel(const __grid_constant__ CUtensorMap mapQ, const __grid_consta
                 const int blk = block_at(p, sb0, sb1, it, C::BN);
                 const int st = it % C::NS;
                 const uint32_t ph = (it / C::NS) & 1;
+                int kv_row, kv_slab;                         // (paged cache: one block-table entry per block)
+                kv_coords(p, b, kvh_in_b, kvslab, blk, C::BN, kv_row, kv_slab);
                 ptx::mbar_wait(k_empty + st, ph ^ 1);
                 ptx::mbar_arrive_expect_tx(k_full + st, C::TILE);
-                ptx::tma_load_3d_hint(sK + st * C::TILE, &mapK, k_full + st, 0, blk * C::BN, kvslab, stream_once);
+                ptx::tma_load_3d_hint(sK + st * C::TILE, &mapK, k_full + st, 0, kv_row, kv_slab, stream_once);
                 ptx::mbar_wait(v_empty + st, ph ^ 1);
                 ptx::mbar_arrive_expect_tx(v_full + st, C::TILE);
-                ptx::tma_load_3d_hint(sV + st * C::TILE, &mapV, v_full + st, 0, blk * C::BN, kvslab, stream_once);
+                ptx::tma_load_3d_hint(sV + st * C::TILE, &mapV, v_full + st, 0, kv_row, kv_slab, stream_once);
             }
         }
     } else if (warp == 4) {
@@ -183,7 +186,6 @@ attn_decode_kernel(const __grid_constant__ CUtensorMap mapQ, const __grid_consta
     } else {
         // ================= softmax: thread = key within the block (S^T lane), later = d index (O^T lane) ======
         const uint32_t tlane = tbase + (static_cast<uint32_t>(warp * 32) << 16);
-        const int off = p.Lk - p.Lq;
         const float c_nat = p.sm_scale * p.k_scale[kvslab];     // times q_scale[row] below (per query head)
         float cl2[NVT], m_run[NVT], l_t[NVT];
         int jlim[NVT];
@@ -197,9 +199,7 @@ attn_decode_kernel(const __grid_constant__ CUtensorMap mapQ, const __grid_consta
             m_run[n] = -INFINITY;
             l_t[n] = 0.0f;
             k_run[n] = 0;
-            long long jl = p.causal ? (long long)lq + off : (long long)p.Lk - 1;
-            if (jl > p.Lk - 1) jl = p.Lk - 1;
-            jlim[n] = (n < nv) ? (int)jl : -1;
+            jlim[n] = (n < nv) ? last_visible_key(p, sq, lq) : -1;
         }
         const float log2S = FOLD ? log2f(p.S) : 0.0f;
         // AUX: which query row (if any) belongs to the dumped head; Lq rows of one q head are consecutive n

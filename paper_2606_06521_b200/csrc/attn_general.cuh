@@ -85,20 +85,19 @@ attn_general_kernel(const __grid_constant__ CUtensorMap mapQ, const __grid_const
     const uint32_t tlane = tbase + (static_cast<uint32_t>(warp * 32) << 16);   // this warp's 32 lanes
 
     // ---- block range of this CTA: split range, clipped by the causal diagonal of the tile ----
-    const int sb0 = (int)(((long long)split * p.nb) / p.num_splits);
-    const int sb1 = (int)(((long long)(split + 1) * p.nb) / p.num_splits);
+    const Seq sq = seq_of(p, b, BN);       // this batch element's lengths (variable-length sequences)
+    const int sb0 = (int)(((long long)split * sq.nb) / p.num_splits);
+    const int sb1 = (int)(((long long)(split + 1) * sq.nb) / p.num_splits);
     int blk_hi = sb1;
     if (p.causal) {
-        long long kmax = (long long)qtile * BM + (BM - 1) + (p.Lk - p.Lq);   // last key any row of the tile sees
-        if (kmax > p.Lk - 1) kmax = p.Lk - 1;
+        long long kmax = (long long)qtile * BM + (BM - 1) + (sq.Lk - sq.Lq);   // last key any row of the tile sees
+        if (kmax > sq.Lk - 1) kmax = sq.Lk - 1;
         int lim = kmax < 0 ? 0 : (int)(kmax / BN) + 1;
         if (lim < blk_hi) blk_hi = lim;
     }
+    if (qtile * BM >= sq.Lq) blk_hi = sb0;                 // no row of this tile exists in this batch element
     const int n_iter = blk_hi > sb0 ? blk_hi - sb0 : 0;
-    // last visible key of this thread's row
-    long long jl = p.causal ? (long long)qrow + (p.Lk - p.Lq) : (long long)p.Lk - 1;
-    if (jl > p.Lk - 1) jl = p.Lk - 1;
-    const int jlim = (int)jl;   // may be negative: row sees nothing
+    const int jlim = last_visible_key(p, sq, qrow);        // may be negative: row sees nothing
 
     // softmax scale folded with the dequantisation scales and log2(e)
     float c_nat = p.sm_scale;
@@ -122,8 +121,8 @@ attn_general_kernel(const __grid_constant__ CUtensorMap mapQ, const __grid_const
     int k_run = 0;            // dynamic scale: O in TMEM carries 2^k_run (the exponent of the last block)
     const bool dynamic = (MODE != 0) && p.scale_mode == 1;
     unsigned int uf_sink = 0, uf_other = 0;
-    const bool dump = (MODE != 0) && p.p_codes != nullptr && bh == p.p_bh && qrow < p.Lq;
-    const bool count = (MODE != 0) && p.underflow != nullptr && qrow < p.Lq;
+    const bool dump = (MODE != 0) && p.p_codes != nullptr && bh == p.p_bh && qrow < sq.Lq;
+    const bool count = (MODE != 0) && p.underflow != nullptr && qrow < sq.Lq;
 
     constexpr uint32_t idesc_qk = ptx::make_idesc(C::FMT, C::FMT, ptx::MAJOR_K, ptx::MAJOR_K, BM, BN);
     constexpr uint32_t pfmt = (MODE == 2) ? ptx::FMT_E4M3 : ptx::FMT_BF16;
@@ -136,16 +135,18 @@ attn_general_kernel(const __grid_constant__ CUtensorMap mapQ, const __grid_const
 
         if (tid == 0) {
             // K and V tiles of this block (their previous readers finished: bar_s / bar_o were waited on)
+            int kv_row, kv_slab;
+            kv_coords(p, b, h / (p.Hq / p.Hkv), kvh, blk, BN, kv_row, kv_slab);
             ptx::mbar_arrive_expect_tx(bar_k, NPL * C::KV_PLANE);
             for (int pl = 0; pl < NPL; ++pl)
                 for (int c = 0; c < C::NCH; ++c)
-                    ptx::tma_load_3d(sK + pl * C::KV_PLANE + c * (BN * 128), &mapK, bar_k, c * C::CH, j0,
-                                     pl * p.kv_slabs + kvh);
+                    ptx::tma_load_3d(sK + pl * C::KV_PLANE + c * (BN * 128), &mapK, bar_k, c * C::CH, kv_row,
+                                     pl * p.kv_slabs + kv_slab);
             ptx::mbar_arrive_expect_tx(bar_v, NPL * C::KV_PLANE);
             for (int pl = 0; pl < NPL; ++pl)
                 for (int c = 0; c < C::NCH; ++c)
-                    ptx::tma_load_3d(sV + pl * C::KV_PLANE + c * (BN * 128), &mapV, bar_v, c * C::CH, j0,
-                                     pl * p.kv_slabs + kvh);
+                    ptx::tma_load_3d(sV + pl * C::KV_PLANE + c * (BN * 128), &mapV, bar_v, c * C::CH, kv_row,
+                                     pl * p.kv_slabs + kv_slab);
             if (it == 0) ptx::mbar_wait(bar_q, 0);
             ptx::mbar_wait(bar_k, ph);
             ptx::tc_fence_after();

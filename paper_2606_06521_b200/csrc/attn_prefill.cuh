@@ -37,17 +37,14 @@ struct PrefillKCfg {
 };
 
 // Which blocks of a tile need the mask for some row of the 32-row group `wq`: blocks whose first key index
-// exceeds the returned value (bottom-right causal diagonal, tail of the sequence; reading R15).
-__device__ __forceinline__ int mask_threshold(const FwdParams& p, int row0, int wq) {
-    const long long wvis = p.causal ? (long long)row0 + wq * 32 + (p.Lk - p.Lq) : (long long)p.Lk - 1;
-    long long thr = wvis - 127 < (long long)p.Lk - 128 ? wvis - 127 : (long long)p.Lk - 128;
+// exceeds the returned value (bottom-right causal diagonal, tail of the sequence, rows past the end of a
+// variable-length sequence; reading R15).
+__device__ __forceinline__ int mask_threshold(const FwdParams& p, const Seq& s, int row0, int wq) {
+    if (row0 + wq * 32 + 31 >= s.Lq) return -(1 << 30);        // some row of the group does not exist: always mask
+    const long long wvis = p.causal ? (long long)row0 + wq * 32 + (s.Lk - s.Lq) : (long long)s.Lk - 1;
+    long long thr = wvis - 127 < (long long)s.Lk - 128 ? wvis - 127 : (long long)s.Lk - 128;
     if (thr < -(1ll << 30)) thr = -(1ll << 30);
     return (int)thr;
-}
-__device__ __forceinline__ int last_visible_key(const FwdParams& p, int qrow) {
-    long long jl = p.causal ? (long long)qrow + (p.Lk - p.Lq) : (long long)p.Lk - 1;
-    if (jl > p.Lk - 1) jl = p.Lk - 1;
-    return (int)jl;       // negative: the row sees no key
 }
 
 // What a max warp publishes per (tile, block, row) for the exp warps: the exponent offset of line 7,
@@ -65,8 +62,9 @@ __device__ __forceinline__ void prefill_max_warp(const FwdParams& p, int t, int 
     const uint32_t tlane = tbase + (static_cast<uint32_t>(wq * 32) << 16);
     const uint32_t tS = tlane + C::TM_S + t * 128, tO = tlane + C::TM_O + t * 128;
     const int rl = wq * 32 + lane;
-    const int jlim = last_visible_key(p, row0 + rl);
-    const int mask_from = mask_threshold(p, row0, wq);
+    const Seq sq = seq_of(p, bh / p.Hq, 128);
+    const int jlim = last_visible_key(p, sq, row0 + rl);
+    const int mask_from = mask_threshold(p, sq, row0, wq);
     float c_nat = p.sm_scale;
     if constexpr (EB == 1) c_nat *= p.q_scale[bh] * p.k_scale[kvh];
     const float cl2 = c_nat * LOG2E;
@@ -190,6 +188,7 @@ __device__ __forceinline__ void prefill_exp_warp(const FwdParams& p, int wq, int
     const float cl2 = c_nat * LOG2E;
     const uint64_t cl2_2 = ptx::pack2(cl2, cl2), s_2 = ptx::pack2(p.S, p.S);
 
+    const Seq sq = seq_of(p, bh / p.Hq, 128);
     int jlim[2], first[2], mask_from[2];
     uint8_t* dump_row[2];     // AUX: this row of the P dump (fp8attn_stats.p_codes), else null
     uint32_t uf_sink = 0, uf_other = 0;   // AUX: zero codes among visible non-sink keys (sink block / other blocks)
@@ -197,10 +196,10 @@ __device__ __forceinline__ void prefill_exp_warp(const FwdParams& p, int wq, int
 #pragma unroll
     for (int t = 0; t < 2; ++t) {
         const int row0 = (pair * 2 + t) * BM;
-        jlim[t] = last_visible_key(p, row0 + rl);
-        mask_from[t] = mask_threshold(p, row0, wq);
+        jlim[t] = last_visible_key(p, sq, row0 + rl);
+        mask_from[t] = mask_threshold(p, sq, row0, wq);
         first[t] = (p.kv_order == 0) ? 0 : n_it - n_tile[t];
-        dump_row[t] = (AUX && p.p_codes != nullptr && bh == p.p_bh && row0 + rl < p.Lq)
+        dump_row[t] = (AUX && p.p_codes != nullptr && bh == p.p_bh && row0 + rl < sq.Lq)
                           ? p.p_codes + (size_t)(row0 + rl) * p.Lk
                           : nullptr;
     }
@@ -247,7 +246,7 @@ __device__ __forceinline__ void prefill_exp_warp(const FwdParams& p, int wq, int
             // l = 0 in the epilogue)
             // AUX: the counter this block adds to (blocks that hold a sink key / all others); rows >= Lq do not
             // exist and are not counted
-            uint32_t* const uf = (AUX && p.underflow != nullptr && (pair * 2 + t) * BM + rl < p.Lq)
+            uint32_t* const uf = (AUX && p.underflow != nullptr && (pair * 2 + t) * BM + rl < sq.Lq)
                                      ? (sink_in_range(p, j0, 128) ? &uf_sink : &uf_other)
                                      : nullptr;
             p_quarter<EB, FOLD, CK::NPOLY, AUX>(r, tS, 2 * half, j0, jlim[t], cl2_2, negm_2, s_2, sum_a, sum_b,
@@ -392,17 +391,18 @@ attn_prefill_kernel(const __grid_constant__ CUtensorMap mapQ, const __grid_const
     const int b = bh / p.Hq, h = bh % p.Hq;
     const int kvh = b * p.Hkv + h / (p.Hq / p.Hkv);
 
-    // visible block count of each tile (bottom-right causal, reading R15)
+    // visible block count of each tile (bottom-right causal, reading R15; this batch element's lengths)
+    const Seq sq = seq_of(p, b, C::BN);
     int n_tile[2];
 #pragma unroll
     for (int t = 0; t < 2; ++t) {
         const long long r0 = (long long)(pair * 2 + t) * BM;
         int n = 0;
-        if (r0 < p.Lq) {
-            n = p.nb;
+        if (r0 < sq.Lq) {
+            n = sq.nb;
             if (p.causal) {
-                long long kmax = r0 + (BM - 1) + (p.Lk - p.Lq);
-                if (kmax > p.Lk - 1) kmax = p.Lk - 1;
+                long long kmax = r0 + (BM - 1) + (sq.Lk - sq.Lq);
+                if (kmax > sq.Lk - 1) kmax = sq.Lk - 1;
                 n = kmax < 0 ? 0 : (int)(kmax / C::BN) + 1;
             }
         }
@@ -465,16 +465,18 @@ attn_prefill_kernel(const __grid_constant__ CUtensorMap mapQ, const __grid_const
                     const int blk = (p.kv_order == 0) ? it : n_it - 1 - it;
                     const int st = it % C::NS;
                     const uint32_t ph = (it / C::NS) & 1;
+                    int kv_row, kv_slab;                     // (paged cache: one block-table entry per block)
+                    kv_coords(p, b, h / (p.Hq / p.Hkv), kvh, blk, C::BN, kv_row, kv_slab);
                     ptx::mbar_wait(k_empty + st, ph ^ 1);
                     ptx::mbar_arrive_expect_tx(k_full + st, C::TILE);
                     for (int c = 0; c < C::NCH; ++c)
                         ptx::tma_load_3d(sK + st * C::TILE + c * (128 * 128), &mapK, k_full + st, c * C::CH,
-                                         blk * C::BN, kvh);
+                                         kv_row, kv_slab);
                     ptx::mbar_wait(v_empty + st, ph ^ 1);
                     ptx::mbar_arrive_expect_tx(v_full + st, C::TILE);
                     for (int c = 0; c < C::NCH; ++c)
                         ptx::tma_load_3d(sV + st * C::TILE + c * (128 * 128), &mapV, v_full + st, c * C::CH,
-                                         blk * C::BN, kvh);
+                                         kv_row, kv_slab);
                 }
             }
         } else if (warp < 18 && n_tile[warp - 16] > 0) {

@@ -31,7 +31,45 @@ struct FwdParams {
     int o_bf16;
     int n_sinkpos;           // -1: the sink keys are the first n_sink keys; else sink_pos[0 .. n_sinkpos) (ascending)
     int sink_pos[MAX_SINKS];
+    const int* seqlens_q;    // [B] or null
+    const int* seqlens_k;    // [B] or null
+    const int* block_table;  // [B, max_pages] or null: k, v are page pools [num_pages, Hkv, page_size, d]
+    int page_size, max_pages;
 };
+
+// ---- per-batch-element geometry (variable-length sequences) and the address of a KV block (paged cache) ----
+struct Seq {
+    int Lq, Lk, nb;          // query rows, keys and KV blocks of this batch element
+};
+__device__ __forceinline__ Seq seq_of(const FwdParams& p, int b, int bn) {
+    Seq s{p.Lq, p.Lk, p.nb};
+    if (p.seqlens_q != nullptr) s.Lq = min(p.Lq, max(0, p.seqlens_q[b]));
+    if (p.seqlens_k != nullptr) {
+        s.Lk = min(p.Lk, max(0, p.seqlens_k[b]));
+        s.nb = (s.Lk + bn - 1) / bn;
+    }
+    return s;
+}
+// Last key row `qrow` sees (bottom-right aligned causal mask, reading R15); negative: it sees no key.
+__device__ __forceinline__ int last_visible_key(const FwdParams& p, const Seq& s, int qrow) {
+    if (qrow >= s.Lq) return -1;
+    long long jl = p.causal ? (long long)qrow + (s.Lk - s.Lq) : (long long)s.Lk - 1;
+    if (jl > s.Lk - 1) jl = s.Lk - 1;
+    return jl < -1 ? -1 : (int)jl;
+}
+// TMA coordinates (row, slab) of KV block `blk` of kv head `kvh_in_b` of batch element b (kvslab = b * Hkv + kvh_in_b)
+__device__ __forceinline__ void kv_coords(const FwdParams& p, int b, int kvh_in_b, int kvslab, int blk, int bn, int& row,
+                                          int& slab) {
+    if (p.block_table == nullptr) {
+        row = blk * bn;
+        slab = kvslab;
+    } else {
+        const int key0 = blk * bn;
+        const int page = p.block_table[(long long)b * p.max_pages + key0 / p.page_size];
+        row = key0 % p.page_size;
+        slab = page * p.Hkv + kvh_in_b;
+    }
+}
 
 // ---- sink keys (underflow classification, Prop. 1 / PAPER.md:443) and the block order (Alg. 1 line 2) ----
 __device__ __forceinline__ bool sink_in_range(const FwdParams& p, int j0, int n) {     // a sink key in [j0, j0 + n)?

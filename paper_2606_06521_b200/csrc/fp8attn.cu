@@ -337,6 +337,12 @@ int validate_args(const void* q, const void* k, const void* v, const void* o, in
     if (stats && (stats->kernel < 0 || stats->kernel > 3 || stats->reserved1 != 0)) return FP8ATTN_E_MODE;
     if (stats && (stats->scale_mode < 0 || stats->scale_mode > 1 || stats->o_dtype < 0 || stats->o_dtype > 1)) return FP8ATTN_E_MODE;
     if (stats && stats->scale_mode == FP8ATTN_SCALE_DYNAMIC && pm == FP8ATTN_MODE_NOCAST) return FP8ATTN_E_MODE;
+    if (stats && stats->reserved2 != 0) return FP8ATTN_E_MODE;
+    if (stats && stats->block_table) {
+        if (stats->page_size < 1 || stats->max_pages < 1 || stats->num_pages < 1) return FP8ATTN_E_SHAPE;
+        if ((long long)stats->max_pages * stats->page_size < Lk) return FP8ATTN_E_SHAPE;
+        if (dt == 0) return FP8ATTN_E_UNSUPPORTED;            // FP32 planes of a page pool: not built
+    }
     if (stats && stats->n_sink < 0) return FP8ATTN_E_SHAPE;
     if (stats && stats->sink_pos) {
         if (stats->n_sink < 1 || stats->n_sink > FP8ATTN_MAX_SINKS) return FP8ATTN_E_SHAPE;
@@ -471,10 +477,17 @@ int fp8attn_fwd(const void* q, const void* k, const void* v, void* o, int B, int
         q_scale = qsc;
     }
 
+    const bool paged = stats && stats->block_table;
+    if (paged && stats->page_size % bn != 0) return FP8ATTN_E_UNSUPPORTED;    // a KV block must not straddle pages
     CUtensorMap mq, mk, mv;
     if (int rc = make_map(&mq, qs, eb, npl * q_slabs, Lq, d, BM)) return rc;
-    if (int rc = make_map(&mk, ks, eb, npl * kv_slabs, Lk, d, bn)) return rc;
-    if (int rc = make_map(&mv, vs, eb, npl * kv_slabs, Lk, d, bn)) return rc;
+    if (paged) {       // k, v are page pools [num_pages, Hkv, page_size, d]: slab = page * Hkv + kv head
+        if (int rc = make_map(&mk, ks, eb, (long long)stats->num_pages * Hkv, stats->page_size, d, bn)) return rc;
+        if (int rc = make_map(&mv, vs, eb, (long long)stats->num_pages * Hkv, stats->page_size, d, bn)) return rc;
+    } else {
+        if (int rc = make_map(&mk, ks, eb, npl * kv_slabs, Lk, d, bn)) return rc;
+        if (int rc = make_map(&mv, vs, eb, npl * kv_slabs, Lk, d, bn)) return rc;
+    }
 
     FwdParams p;
     memset(&p, 0, sizeof p);
@@ -499,6 +512,12 @@ int fp8attn_fwd(const void* q, const void* k, const void* v, void* o, int B, int
         for (int i = 0; i < stats->n_sink; ++i) p.sink_pos[i] = stats->sink_pos[i];
     }
     const bool dynamic = p.scale_mode == 1;
+    p.seqlens_q = stats ? stats->seqlens_q : nullptr;
+    p.seqlens_k = stats ? stats->seqlens_k : nullptr;
+    p.block_table = paged ? stats->block_table : nullptr;
+    p.page_size = paged ? stats->page_size : 0;
+    p.max_pages = paged ? stats->max_pages : 0;
+    const bool varlen = p.seqlens_q || p.seqlens_k || paged;
     p.num_splits = ns;
     p.nb = nb;
     p.q_slabs = (int)q_slabs;
@@ -522,7 +541,7 @@ int fp8attn_fwd(const void* q, const void* k, const void* v, void* o, int B, int
     // inputs, the no-cast mode, d = 64, prefill with splits -- runs on the general kernel.
     // (not built into the prefill kernels: the sink-blocks-last order; the dynamic scale with Bn = 64)
     const bool prefill_ok = d == 128 && ns == 1 && npl == 1 && pm != 0 && dt != 3 && kv_order != FP8ATTN_ORDER_SINK_LAST &&
-                            !(dynamic && bn == 64);
+                            !(dynamic && bn == 64) && !(varlen && bn == 64);
     if (want_kernel == 2 && !prefill_ok) return FP8ATTN_E_UNSUPPORTED;
     // (automatic selection keeps prefill-shaped calls that ask for the P dump or the underflow counters on the
     // general kernel, whose serial schedule is the reference for them; stats->kernel = 2 takes the statistics
@@ -581,6 +600,7 @@ int fp8attn_fwd(const void* q, const void* k, const void* v, void* o, int B, int
 int fp8attn_fwd_host(const void* q, const void* k, const void* v, void* o, int B, int Hq, int Hkv, int Lq, int Lk,
                      int d, int causal, float S, int kv_order, int mode, fp8attn_stats* stats) {
     if (int rc = validate_args(q, k, v, o, B, Hq, Hkv, Lq, Lk, d, S, kv_order, mode, stats)) return rc;
+    if (stats && (stats->seqlens_q || stats->seqlens_k || stats->block_table)) return FP8ATTN_E_UNSUPPORTED;
     if (int rc = check_device()) return rc;
     const int dt = (mode >> 8) & 0xF;
     const size_t ebq = (dt == 0) ? 4 : (dt == 2 ? 1 : 2);

@@ -32,6 +32,8 @@ class Stats(C.Structure):
         ("stream", C.c_void_p), ("p_codes", C.c_void_p),
         ("p_batch", C.c_int32), ("p_head", C.c_int32),
         ("sink_pos", C.c_void_p), ("o_dtype", C.c_int32), ("reserved1", C.c_int32),
+        ("seqlens_q", C.c_void_p), ("seqlens_k", C.c_void_p), ("block_table", C.c_void_p),
+        ("page_size", C.c_int32), ("max_pages", C.c_int32), ("num_pages", C.c_int32), ("reserved2", C.c_int32),
         ("row_max", C.c_void_p), ("row_sum", C.c_void_p), ("underflow", C.c_void_p),
         ("block_m_used", C.c_int32), ("block_n_used", C.c_int32), ("num_splits_used", C.c_int32),
         ("split_bounds", C.c_int32 * (MAX_SPLITS + 1)),
@@ -143,19 +145,30 @@ def _dtype_code(q, k):
 def fwd(q, k, v, *, causal: bool, S: float, kv_order: int, mode: int, n_sink: int = 4,
         block_n: int = 0, num_splits: int = 0, kernel: int = 0, q_scale=None, k_scale=None, v_scale=None,
         want_stats: bool = False, want_underflow: Optional[bool] = None, dump_head=None, out=None,
-        stream=None, scale_mode: int = 0, sink_pos=None, out_dtype=None) -> FwdResult:
+        stream=None, scale_mode: int = 0, sink_pos=None, out_dtype=None, seqlens_q=None, seqlens_k=None,
+        block_table=None, Lk=None) -> FwdResult:
     """fp8attn_fwd on CUDA tensors q [B,Hq,Lq,d], k/v [B,Hkv,Lk,d] (contiguous).  `mode` is the
     P mode (0 no-cast, 1 isolation, 2 FP8); the input dtype bits are derived from the tensors.
     `dump_head=(b,h)` returns the E4M3 code of every P of that head.  `kernel` requests a kernel
     family (0 automatic, 1 general, 2 prefill, 3 decode).  `scale_mode=1`: dynamic per-(row, block) 2^k scale;
-    `sink_pos`: ascending key indices of the sink keys (replaces n_sink); `out_dtype=torch.bfloat16`: BF16 output."""
+    `sink_pos`: ascending key indices of the sink keys (replaces n_sink); `out_dtype=torch.bfloat16`: BF16 output.
+    `seqlens_q` / `seqlens_k`: int32 CUDA tensors [B] (variable-length sequences in the padded layout).
+    `block_table`: int32 CUDA tensor [B, max_pages]; k, v are then page pools [num_pages, Hkv, page_size, d] and
+    `Lk` (the longest sequence, default max_pages * page_size) must be given."""
     for t in (q, k, v):
         if not (t.is_cuda and t.is_contiguous() and t.dim() == 4):
             raise ValueError("q, k, v must be contiguous 4-D CUDA tensors")
     B, Hq, Lq, d = q.shape
-    Bk, Hkv, Lk, dk = k.shape
-    if (Bk, dk) != (B, d) or v.shape != k.shape:
-        raise ValueError("shape mismatch between q, k, v")
+    if block_table is not None:
+        n_pages, Hkv, page_size, dk = k.shape
+        max_pages = block_table.shape[1]
+        Lk = max_pages * page_size if Lk is None else int(Lk)
+        if dk != d or v.shape != k.shape or block_table.shape[0] != B or block_table.dtype != torch.int32:
+            raise ValueError("paged k, v must be [num_pages, Hkv, page_size, d] and block_table int32 [B, max_pages]")
+    else:
+        Bk, Hkv, Lk, dk = k.shape
+        if (Bk, dk) != (B, d) or v.shape != k.shape:
+            raise ValueError("shape mismatch between q, k, v")
     if out is not None:
         out_dtype = out.dtype
     out_dtype = torch.float32 if out_dtype is None else out_dtype
@@ -170,6 +183,13 @@ def fwd(q, k, v, *, causal: bool, S: float, kv_order: int, mode: int, n_sink: in
     st.stream = _stream_ptr(stream)
     keep = []
     _set_sinks(st, sink_pos, keep)
+    for name, t in (("seqlens_q", seqlens_q), ("seqlens_k", seqlens_k), ("block_table", block_table)):
+        if t is not None:
+            t = t.to(device=q.device, dtype=torch.int32).contiguous()
+            keep.append(t)
+            setattr(st, name, t.data_ptr())
+    if block_table is not None:
+        st.page_size, st.max_pages, st.num_pages = int(page_size), int(max_pages), int(n_pages)
     for name, t in (("q_scale", q_scale), ("k_scale", k_scale), ("v_scale", v_scale)):
         if t is not None:
             t = t.to(device=q.device, dtype=torch.float32).contiguous()
