@@ -234,12 +234,13 @@ attn_general_kernel(const __grid_constant__ CUtensorMap mapQ, const __grid_const
                 for (int e = 0; e < 32; e += 2)
                     pair[e / 2] = ptx::cvt_e4m3x2(pr[e] * S_blk, pr[e + 1] * S_blk);   // line 9
                 if (count || dump) {
+                    const uint32_t sinks = sink_mask32(p, j0 + cb * 32);
 #pragma unroll
                     for (int e = 0; e < 32; ++e) {
                         const int j = j0 + cb * 32 + e;
                         const uint32_t code = (pair[e / 2] >> ((e & 1) * 8)) & 0xFFu;
                         const bool vis = j <= jlim;
-                        if (count && vis && code == 0 && !is_sink_key(p, j)) {
+                        if (count && vis && code == 0 && !((sinks >> e) & 1u)) {
                             if (sink_blk) ++uf_sink; else ++uf_other;
                         }
                         if (dump && j < p.Lk) p.p_codes[(size_t)qrow * p.Lk + j] = vis ? (uint8_t)code : (uint8_t)0xFF;

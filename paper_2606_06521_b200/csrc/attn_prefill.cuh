@@ -226,6 +226,9 @@ __device__ __forceinline__ void prefill_exp_warp(const FwdParams& p, int wq, int
             const uint32_t tS = tlane + C::TM_S + t * 128;
             // ---- the running max of block c is published (which implies S(c) is complete): this warp's 64
             // logits of the row, loaded once ----
+            // ---- the running max of block c is published (which implies S(c) is complete): this warp's 64
+            // logits of the row, loaded once.  (Waiting for S first, loading, then waiting for the max -- two
+            // barrier round trips -- measured 8 % slower than this single wait.) ----
             uint32_t r[64];
             if (probed_tile != t || !ptx::mbar_probe_result()) ptx::mbar_wait(m_full + 4 * t + wq, c & 1);
             probed_tile = -1;
@@ -499,10 +502,9 @@ attn_prefill_kernel(const __grid_constant__ CUtensorMap mapQ, const __grid_const
             uint64_t* const pf = p_full + 2 * t;
 
             // S_t = Q_t K^T on ring iteration it
+            // (the caller has waited for the K tile of ring iteration it: k_full)
             auto qk_block = [&](const int it) {
                 const int st = it % C::NS;
-                ptx::mbar_wait(k_full + st, (it / C::NS) & 1);
-                ptx::tc_fence_after();
                 if (leader) {
                     const uint32_t b0 = k_lo + st * (C::TILE >> 4);
 #pragma unroll
@@ -533,6 +535,8 @@ attn_prefill_kernel(const __grid_constant__ CUtensorMap mapQ, const __grid_const
 
             ptx::mbar_wait(q_full + t, 0);
             ptx::tc_fence_after();
+            ptx::mbar_wait(k_full + first % C::NS, (first / C::NS) & 1);
+            ptx::tc_fence_after();
             qk_block(first);
             for (int c = 0; c < n_t; ++c) {
                 const int it = c + first;
@@ -545,6 +549,9 @@ attn_prefill_kernel(const __grid_constant__ CUtensorMap mapQ, const __grid_const
                 ptx::tc_fence_after();
                 pv_quarter(0, it, c > 0 ? 1u : 0u);
                 pv_quarter(2, it, 1u);
+                // everything between the last P quarter and S(c+1) is on the chain the exp warps wait for (an mbarrier
+                // wait costs 150-300 cycles even when the phase is complete): the next K tile is waited for here
+                if (has_next) ptx::mbar_wait(k_full + (it + 1) % C::NS, ((it + 1) / C::NS) & 1);
                 ptx::mbar_wait(pf + 1, c & 1);
                 ptx::tc_fence_after();
                 pv_quarter(1, it, 1u);

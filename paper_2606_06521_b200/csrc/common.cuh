@@ -75,10 +75,25 @@ __device__ __forceinline__ void kv_coords(const FwdParams& p, int b, int kvh_in_
 __device__ __forceinline__ bool sink_in_range(const FwdParams& p, int j0, int n) {     // a sink key in [j0, j0 + n)?
     if (p.n_sinkpos < 0) return j0 < p.n_sink;
     bool any = false;
+#pragma unroll 1
     for (int s = 0; s < p.n_sinkpos; ++s) any |= (p.sink_pos[s] >= j0 && p.sink_pos[s] < j0 + n);
     return any;
 }
 __device__ __forceinline__ bool is_sink_key(const FwdParams& p, int j) { return sink_in_range(p, j, 1); }
+// bit e set = key j0 + e is a sink key (e < 32)
+__device__ __forceinline__ uint32_t sink_mask32(const FwdParams& p, int j0) {
+    if (p.n_sinkpos < 0) {
+        const int n = p.n_sink - j0;
+        return n <= 0 ? 0u : (n >= 32 ? 0xFFFFFFFFu : ((1u << n) - 1u));
+    }
+    uint32_t m = 0;
+#pragma unroll 1
+    for (int s = 0; s < p.n_sinkpos; ++s) {
+        const int e = p.sink_pos[s] - j0;
+        if (e >= 0 && e < 32) m |= 1u << e;
+    }
+    return m;
+}
 // Block visited at step `step` of the block range [b0, b1): forward, reverse, or sink blocks last (the blocks
 // without a sink key in descending order, then those with one, in descending order; reading R27).
 __device__ __forceinline__ int block_at(const FwdParams& p, int b0, int b1, int step, int bn) {

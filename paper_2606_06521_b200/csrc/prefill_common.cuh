@@ -135,8 +135,8 @@ __device__ __forceinline__ void chunk_statistics(const uint32_t* w, int jq, int 
                                                  const FwdParams& p) {
     constexpr int NW = 8 * EB;      // words of the chunk
     if (dump_row == nullptr && uf == nullptr) return;
-    const bool has_sink = sink_in_range(p, jq, 32);
-    if (dump_row == nullptr && !has_sink && jq + 31 <= jlim) {
+    const uint32_t sinks = sink_mask32(p, jq);        // which keys of the chunk are sink keys
+    if (dump_row == nullptr && sinks == 0u && jq + 31 <= jlim) {
         // every key of the chunk is visible and none is a sink: count the zero codes a word at a time
         uint32_t zeros = 0;
 #pragma unroll
@@ -158,7 +158,7 @@ __device__ __forceinline__ void chunk_statistics(const uint32_t* w, int jq, int 
         }
         const bool vis = jq + e <= jlim;
         if (vis && dump_row != nullptr) dump_row[jq + e] = (uint8_t)code;
-        if (vis && code == 0 && !(has_sink && is_sink_key(p, jq + e))) ++zeros;
+        if (vis && code == 0 && !((sinks >> e) & 1u)) ++zeros;
     }
     if (uf != nullptr) *uf += zeros;
 }

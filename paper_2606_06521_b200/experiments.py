@@ -1,6 +1,6 @@
 """The paper's experiment grid on the CUDA path.
 
-    python -m paper_2606_06521_b200.experiments --exp table1|exp1|exp2|ttest|cfg2 [--seeds K]
+    python -m paper_2606_06521_b200.experiments --exp table1|exp1|exp2|ttest|cfg2|dynamic [--seeds K]
 
 Every number is computed by `fp8attn_fwd` on a B200: the P-cast runs in isolation mode (FP32 Q, K, V; P cast
 to E4M3 at scale S) and the error is taken against the no-cast mode of the same library
@@ -13,6 +13,8 @@ Set-ups (all synthetic, as in the paper; inputs from `workloads.sink_qkv`):
   exp1    PAPER.md:355-362  Delta in [4,13], N=4096, d=128, q_len=32, B=64, k_sink=4; the five configurations
   exp2    PAPER.md:366, 378-388 (Table 2)  Delta=7, N in {512 .. 16384}
   ttest   PAPER.md:474-485 (App. B)  paired t statistic of MSE(Fwd+256) - MSE(Rev+256) over instances
+  dynamic PAPER.md:435  the Exp. 1 grid with the dynamic per-(row, block) power-of-two scale (scale_mode = 1) next
+          to the static S = 256, both orders: MSE and the share of non-sink P values that cast to zero
   cfg2    BASELINE.json configs[1]  B=1, H=8, L=2048, d=128, Delta = 0 .. 14 in steps of 0.5, S in {1,16,256,448}, both
           orders: MSE and underflow fraction next to Eq. 7.  (The same sweep held against the CPU
           oracle point by point is tests/cfg2_sweep.py; its table is profiles/cfg2_sweep.md.)
@@ -168,9 +170,30 @@ def cfg2(deltas=tuple(0.5 * i for i in range(29)), scales=(1.0, 16.0, 256.0, 448
     return out
 
 
+def dynamic(seeds: int = 20, deltas=tuple(range(4, 14)), n_keys: int = 4096):
+    out = []
+    for d in deltas:
+        acc = {}
+        for s in range(seeds):
+            inst = Instance(n_keys, d, s)
+            ref = inst.reference()
+            for order, oname in ((0, "Fwd"), (1, "Rev")):
+                for sm, sname in ((0, "S=256"), (1, "dynamic")):
+                    r = fa.fwd(inst.q, inst.k, inst.v, causal=False, S=256.0, kv_order=order, mode=1, block_n=BLOCK,
+                               want_stats=True, scale_mode=sm)
+                    uf = r.underflow.cpu().numpy().astype(np.float64).sum()
+                    a = acc.setdefault(f"{oname} {sname}", [[], []])
+                    a[0].append(float(((r.o.double() - ref) ** 2).mean().item()))
+                    a[1].append(uf / (B * LQ * (n_keys - 4)))
+        out.append({"exp": "dynamic", "delta": d, "n_keys": n_keys, "seeds": seeds,
+                    "mse": {c: float(np.mean(v[0])) for c, v in acc.items()},
+                    "zeroed": {c: float(np.mean(v[1])) for c, v in acc.items()}})
+    return out
+
+
 def main(argv=None):
     ap = argparse.ArgumentParser(description=__doc__, formatter_class=argparse.RawDescriptionHelpFormatter)
-    ap.add_argument("--exp", required=True, choices=["table1", "exp1", "exp2", "ttest", "cfg2"])
+    ap.add_argument("--exp", required=True, choices=["table1", "exp1", "exp2", "ttest", "cfg2", "dynamic"])
     ap.add_argument("--seeds", type=int, default=0, help="seeds / instances (0: the paper's count)")
     a = ap.parse_args(argv)
     if a.exp == "table1":
@@ -181,6 +204,8 @@ def main(argv=None):
         rows = exp2(a.seeds or 20)
     elif a.exp == "cfg2":
         rows = cfg2()
+    elif a.exp == "dynamic":
+        rows = dynamic(a.seeds or 20)
     else:
         rows = ttest(a.seeds or 100)
     for r in rows:
