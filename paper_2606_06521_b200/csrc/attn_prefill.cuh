@@ -225,8 +225,6 @@ __device__ __forceinline__ void prefill_exp_warp(const FwdParams& p, int wq, int
             const bool mask = j0 > mask_from[t];
             const uint32_t tS = tlane + C::TM_S + t * 128;
             // ---- the running max of block c is published (which implies S(c) is complete): this warp's 64
-            // logits of the row, loaded once ----
-            // ---- the running max of block c is published (which implies S(c) is complete): this warp's 64
             // logits of the row, loaded once.  (Waiting for S first, loading, then waiting for the max -- two
             // barrier round trips -- measured 8 % slower than this single wait.) ----
             uint32_t r[64];
