@@ -42,6 +42,21 @@ WORKLOADS = {
 }
 
 
+# tiling the library uses for each workload (block_m, block_n, num_splits); the reference arm mirrors it so that both
+# arms describe the same configuration (the oracle takes block_n and the split bounds from here)
+TILING = {"cfg3": (256, 128, 1), "cfg4-fp8": (256, 128, 1), "cfg4-bf16": (256, 128, 1), "cfg5": (128, 128, 4)}
+
+
+def config_of(workload, block_m, block_n, num_splits):
+    cfg_name, kind, mode, S, order = WORKLOADS[workload]
+    cfg = W.CONFIGS[cfg_name]
+    return {"workload": f"{workload}: B={cfg.B} Hq={cfg.Hq} Hkv={cfg.Hkv} Lq={cfg.Lq} Lk={cfg.Lk} d={cfg.d} "
+                        f"causal={cfg.causal} Delta={cfg.delta} S={S} order={'reverse' if order else 'forward'} "
+                        f"mode={mode} inputs={kind}",
+            "block_m": block_m, "block_n": block_n, "num_splits": num_splits,
+            "l2": "inputs larger than L2 (no flush)", "sharding": "one replica of the workload per GPU"}
+
+
 def load_peaks():
     """Measured peaks (driver-written MEASURED_PEAKS.json) or the profiling guide's fallback, plus the dense FP8
     GEMM peak measured on this pool in round 2 (profiles/fp8_peak.json; SURVEY.md 8(d) "FP8 peak -- measure")."""
@@ -353,11 +368,7 @@ def run_ours(args, rank, world, dev):
         "ms_per_step": ms, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
         "dtype": "e4m3 (fp32 accumulate)" if mode == 2 else "bf16 (fp32 accumulate), P cast to e4m3",
         "data": "synthetic",
-        "config": {"workload": f"{args.workload}: B={cfg.B} Hq={cfg.Hq} Hkv={cfg.Hkv} Lq={cfg.Lq} Lk={cfg.Lk} d={cfg.d} "
-                               f"causal={cfg.causal} Delta={cfg.delta} S={S} order={'reverse' if order else 'forward'} "
-                               f"mode={mode} inputs={kind}",
-                   "block_m": r.block_m, "block_n": r.block_n, "num_splits": r.num_splits,
-                   "l2": "inputs larger than L2 (no flush)", "sharding": "one replica of the workload per GPU"},
+        "config": config_of(args.workload, r.block_m, r.block_n, r.num_splits),
         "clocks": clocks, "e2e": e2e, "gpu_launches": int(r.n_launches * args.steps),
         "roofline": roof,
     }
@@ -383,7 +394,9 @@ class OracleSample:
         g = cfg.Hq // cfg.Hkv
         self.q = q[None, kv_head * g:(kv_head + 1) * g]       # the q heads of this kv head
         self.k, self.v = k[None, kv_head:kv_head + 1], v[None, kv_head:kv_head + 1]
-        self.block_n = 128
+        _, self.block_n, ns = TILING[workload]
+        nb = (cfg.Lk + self.block_n - 1) // self.block_n
+        self.split_bounds = [(s * nb) // ns for s in range(ns + 1)] if ns > 1 else None
         if self.kind == "bf16":
             self.q, self.k, self.v = (W.to_bf16_bits(a) for a in (self.q, self.k, self.v))
             self.dt, self.sc = oracle.DT_BF16, {}
@@ -416,7 +429,8 @@ class OracleSample:
         rows = np.sort(self.rng.choice(self.n_total, size=n_rows, replace=False)).astype(np.int64)
         t0 = time.perf_counter()
         res = self.oracle.attention_fwd(self.q, self.k, self.v, causal=self.cfg.causal, S=self.S, kv_order=self.order,
-                                        mode=self.mode, in_dtype=self.dt, block_n=self.block_n, rows=rows, **self.sc)
+                                        mode=self.mode, in_dtype=self.dt, block_n=self.block_n, rows=rows,
+                                        split_bounds=self.split_bounds, **self.sc)
         el = time.perf_counter() - t0
         return self.amount(rows), el, res.n_threads, n_rows
 
@@ -467,12 +481,9 @@ def run_reference(args):
         "value": value, "unit": unit, "n_gpus": args.gpus, "steps": args.steps, "warmup": max(args.warmup, 1),
         "ms_per_step": ms, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
         "dtype": "f64 (CPU oracle; E4M3 rounding by table)", "data": "synthetic",
-        "config": {"workload": f"{args.workload}: B={cfg.B} Hq={cfg.Hq} Hkv={cfg.Hkv} Lq={cfg.Lq} Lk={cfg.Lk} d={cfg.d} "
-                               f"causal={cfg.causal} Delta={cfg.delta} S={S} order={'reverse' if order else 'forward'} "
-                               f"mode={mode} inputs={kind}",
-                   "sample_rows_per_step": n},
+        "config": config_of(args.workload, *TILING[args.workload]),
         "cpu_baseline": {"value": value, "unit": unit, "cores": threads, "kind": "oracle",
-                         "sample": f"each step = {n} random query rows of (b=0, kv head 0) of {args.workload}"},
+                         "sample": f"each step = {n} random query rows of (b=0, kv head 0) of {args.workload}, all visible keys"},
         "e2e": {"value": value, "unit": unit, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
         "gpu_launches": 0,
     }
@@ -548,9 +559,7 @@ def run_ours_extra(args, dev):
     out = {"value": amount / (ms * 1e-3), "unit": unit, "ms_per_step": ms, "steps": args.steps, "kernel_id": r.kernel_id,
            "num_splits": r.num_splits, "block_n": r.block_n, "gpu_launches_per_step": r.n_launches,
            "dtype": "e4m3 (fp32 accumulate)" if mode == 2 else "bf16 (fp32 accumulate), P cast to e4m3",
-           "config": {"workload": f"{args.workload}: B={cfg.B} Hq={cfg.Hq} Hkv={cfg.Hkv} Lq={cfg.Lq} Lk={cfg.Lk} d={cfg.d} "
-                                  f"causal={cfg.causal} Delta={cfg.delta} S={S} order={'reverse' if order else 'forward'} "
-                                  f"mode={mode} inputs={kind}"},
+           "config": config_of(args.workload, r.block_m, r.block_n, r.num_splits),
            "clocks": clocks,
            "roofline": roofline_of(args.workload, cfg, mode, bound, amount, float(np.mean(per_step)), r.kernel_id,
                                    load_peaks())}
