@@ -61,8 +61,7 @@ extern "C" {
                                        largest k <= 30 with 2^k * exp(m_loc - m_new) <= 448, i.e.
                                        k_j = floor(log2 448 + (m_new - m_loc) log2 e) in FP32
                                        ("dynamic per-block scale ... constrained to
-                                       2^k"; reading R26).  S is not used.  Modes 1, 2;
-                                       general, decode and Bn = 128 prefill kernels.             */
+                                       2^k"; reading R26).  S is not used.  Modes 1, 2.  */
 
 /* ---- stats->o_dtype ------------------------------------------------------------------ */
 #define FP8ATTN_O_F32  0

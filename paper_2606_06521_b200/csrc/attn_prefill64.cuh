@@ -30,7 +30,7 @@ struct Prefill64Cfg {
     static constexpr int KSTEP = 32 / EB;            // contraction elements per MMA
     static constexpr int TM_S = 0, TM_O = 256;
     static constexpr int N_BARS = 2 + 4 * NS + 4 + 4 + 2 + 2 + 16;
-    static constexpr int SMEM_BYTES = 2 * QTILE + 2 * NS * TILE + 1024 /*align*/ + N_BARS * 8 + 16 + 6144 /*Softmax64Shared*/;
+    static constexpr int SMEM_BYTES = 2 * QTILE + 2 * NS * TILE + 1024 /*align*/ + N_BARS * 8 + 16 + 8192 /*Softmax64Shared*/;
     static constexpr uint32_t KIND = (EB == 1) ? ptx::KIND_F8F6F4 : ptx::KIND_F16;
     static constexpr uint32_t FMT = (EB == 1) ? ptx::FMT_E4M3 : ptx::FMT_BF16;
     static constexpr int THREADS = 608;
@@ -48,8 +48,9 @@ struct Softmax64Shared {
     float m[2][2][128];         // [tile][block parity][row]  running max after that block
     float l[2][2][128];         // [tile][par][row]           final partial row sums
     float mlast[2][2][128];     // [tile][par][row]           the max each partial sum is relative to
+    int kexp[2][2][128];        // [tile][block parity][row]  dynamic scale: exponent of that block (what O carries)
 };
-static_assert(sizeof(Softmax64Shared) == 6144, "SMEM_BYTES accounts for 6144 bytes");
+static_assert(sizeof(Softmax64Shared) == 8192, "SMEM_BYTES accounts for 8192 bytes");
 
 template <int EB, bool FOLD, bool AUX>
 __device__ __forceinline__ void prefill64_softmax(const FwdParams& p, int t, int par, int wq, int lane, uint32_t tbase,
@@ -61,12 +62,14 @@ __device__ __forceinline__ void prefill64_softmax(const FwdParams& p, int t, int
     const uint32_t tS = tlane + C::TM_S + t * 128 + par * 64, tO = tlane + C::TM_O + t * 128;
     const int r = wq * 32 + lane;
     const int qrow = row0 + r;
-    const int off = p.Lk - p.Lq;
-    long long jl = p.causal ? (long long)qrow + off : (long long)p.Lk - 1;
-    if (jl > p.Lk - 1) jl = p.Lk - 1;
-    const int jlim = (int)jl;
-    // last key that every row of this warp sees (blocks reaching past it need the masked path)
-    const long long warp_vis = p.causal ? (long long)(row0 + wq * 32) + off : (long long)p.Lk - 1;
+    const Seq sq = seq_of(p, bh / p.Hq, C::BN);      // this batch element's lengths (variable-length sequences)
+    const int off = sq.Lk - sq.Lq;
+    const int jlim = last_visible_key(p, sq, qrow);
+    // last key that every row of this warp sees (blocks reaching past it need the masked path); a warp with a row
+    // past the end of its sequence always masks
+    const long long warp_vis = (row0 + wq * 32 + 31 >= sq.Lq) ? -1
+                               : (p.causal ? (long long)(row0 + wq * 32) + off : (long long)sq.Lk - 1);
+    const bool dynamic = p.scale_mode == 1;          // reading R26 (the host launches the FOLD instance for it)
     const int bar_id = 1 + t * 4 + wq;            // named barrier of the two warps of these 32 rows
 
     float c_nat = p.sm_scale, vs = 1.0f;
@@ -75,19 +78,20 @@ __device__ __forceinline__ void prefill64_softmax(const FwdParams& p, int t, int
         vs = p.v_scale[kvh];
     }
     const float cl2 = c_nat * LOG2E;
-    const float log2S = FOLD ? log2f(p.S) : 0.0f;   // exact for S = 2^k
+    const float log2S = (FOLD && !dynamic) ? log2f(p.S) : 0.0f;   // exact for S = 2^k
     const uint64_t cl2_2 = ptx::pack2(cl2, cl2), s_2 = ptx::pack2(p.S, p.S);
 
     float m_own = -INFINITY, l_own = 0.0f;   // partial sum of this warp's blocks, relative to m_own; carries S when FOLD
+    int k_own = 0;                           // dynamic: the exponent l_own carries (this warp's last block)
     // statistics instance: this row of the P dump, and the zero codes among visible non-sink keys
-    uint8_t* const dump_row = (AUX && p.p_codes != nullptr && bh == p.p_bh && qrow < p.Lq)
+    uint8_t* const dump_row = (AUX && p.p_codes != nullptr && bh == p.p_bh && qrow < sq.Lq)
                                   ? p.p_codes + (size_t)qrow * p.Lk : nullptr;
-    const bool count = AUX && p.underflow != nullptr && qrow < p.Lq;
+    const bool count = AUX && p.underflow != nullptr && qrow < sq.Lq;
     uint32_t uf_sink = 0, uf_other = 0;
     for (int c = par; c < n_t; c += 2) {
         const int blk = (p.kv_order == 0) ? c : n_t - 1 - c;
         const int j0 = blk * C::BN;
-        const bool mask = (j0 + C::BN - 1 > warp_vis) || (j0 + C::BN > p.Lk);
+        const bool mask = (j0 + C::BN - 1 > warp_vis) || (j0 + C::BN > sq.Lk);
         ptx::mbar_wait(s_full + par, (c >> 1) & 1);
         ptx::tc_fence_after();
         // ---- lines 4-5: block max, running max ----
@@ -115,18 +119,28 @@ __device__ __forceinline__ void prefill64_softmax(const FwdParams& p, int t, int
             mloc = fmaxf(fmaxf(m0, m1), fmaxf(m2, m3));
         }
         float m_prev = -INFINITY;                 // running max after block c-1, from the partner warp
+        int k_prev = 0;                           // dynamic: the exponent O carries after block c-1
         if (c > 0) {
             ptx::mbar_wait(m_full + (par ^ 1), ((c - 1) >> 1) & 1);
             m_prev = sh->m[t][par ^ 1][r];
+            k_prev = sh->kexp[t][par ^ 1][r];
         }
         const float m_new = fmaxf(m_prev, mloc);
+        const int k_new = !dynamic ? 0 : ((mloc == -INFINITY) ? k_prev : dyn_exponent((m_new - mloc) * cl2));
         sh->m[t][par][r] = m_new;
+        sh->kexp[t][par][r] = k_new;
         __syncwarp();
         if (lane == 0) ptx::mbar_arrive(m_full + par);
         const float m_used = (m_new == -INFINITY) ? 0.0f : m_new;
-        const float alpha_o = ptx::ex2_approx((m_prev - m_used) * cl2);   // line 6: what O (state after c-1) is scaled by
-        const float alpha_l = ptx::ex2_approx((m_own - m_used) * cl2);    // the same for this warp's partial sum
-        const float negm = fmaf(-m_used, cl2, log2S);
+        float alpha_o = ptx::ex2_approx((m_prev - m_used) * cl2);   // line 6: what O (state after c-1) is scaled by
+        float alpha_l = ptx::ex2_approx((m_own - m_used) * cl2);    // the same for this warp's partial sum
+        float negm = fmaf(-m_used, cl2, log2S);
+        if (dynamic) {        // 2^k of this block in the exponent of P; O and l are brought from their scales to it
+            negm = fmaf(-m_used, cl2, (float)k_new);
+            alpha_o *= exp2f((float)(k_new - k_prev));
+            alpha_l *= exp2f((float)(k_new - k_own));
+            k_own = k_new;
+        }
         const uint64_t negm_2 = ptx::pack2(negm, negm);
 
         // ---- lines 7-9: P = exp(Z - m), l from the pre-cast P, cast, P -> TMEM over the head of S ----
@@ -187,19 +201,23 @@ __device__ __forceinline__ void prefill64_softmax(const FwdParams& p, int t, int
         }
     }
     // ---- merge the two partial row sums; line 12: O / (S l), statistics ----
-    sh->l[t][par][r] = l_own;
+    // (dynamic scale: each partial sum is first brought to true units, 2^-k_own; O carries the exponent of the last
+    // block, which the warp of that block published)
+    const float own_true = dynamic ? l_own * exp2f((float)-k_own) : l_own;
+    sh->l[t][par][r] = own_true;
     sh->mlast[t][par][r] = m_own;
     asm volatile("bar.sync %0, 64;" ::"r"(bar_id) : "memory");
     const float m_oth = sh->mlast[t][par ^ 1][r], l_oth = sh->l[t][par ^ 1][r];
     const float m_fin = fmaxf(m_own, m_oth);
     const float m_fu = (m_fin == -INFINITY) ? 0.0f : m_fin;
-    const float l_all = l_own * ptx::ex2_approx((m_own - m_fu) * cl2) + l_oth * ptx::ex2_approx((m_oth - m_fu) * cl2);
+    const float l_all = own_true * ptx::ex2_approx((m_own - m_fu) * cl2) + l_oth * ptx::ex2_approx((m_oth - m_fu) * cl2);
+    const float o_carries = (dynamic && n_t > 0) ? exp2f((float)sh->kexp[t][(n_t - 1) & 1][r]) : 1.0f;
     const long long grow = (long long)bh * p.Lq + qrow;
     if (qrow < p.Lq && par == 0) {
         if (p.row_max) p.row_max[grow] = (m_fin == -INFINITY) ? -INFINITY : m_fin * c_nat;
-        if (p.row_sum) p.row_sum[grow] = FOLD ? l_all / p.S : l_all;
+        if (p.row_sum) p.row_sum[grow] = (FOLD && !dynamic) ? l_all / p.S : l_all;
     }
-    const float inv = (l_all > 0.0f) ? (FOLD ? vs / l_all : vs / (p.S * l_all)) : 0.0f;
+    const float inv = (l_all > 0.0f) ? (dynamic ? vs / (o_carries * l_all) : (FOLD ? vs / l_all : vs / (p.S * l_all))) : 0.0f;
     if (n_t > 0) {
         ptx::mbar_wait(o_done, 0);
         ptx::tc_fence_after();
@@ -263,17 +281,18 @@ attn_prefill64_kernel(const __grid_constant__ CUtensorMap mapQ, const __grid_con
     const int b = bh / p.Hq, h = bh % p.Hq;
     const int kvh = b * p.Hkv + h / (p.Hq / p.Hkv);
 
-    // visible block count of each tile (bottom-right causal, reading R15)
+    // visible block count of each tile (bottom-right causal, reading R15; this batch element's lengths)
+    const Seq sq = seq_of(p, b, C::BN);
     int n_tile[2];
 #pragma unroll
     for (int t = 0; t < 2; ++t) {
         const long long r0 = (long long)(pair * 2 + t) * BM;
         int n = 0;
-        if (r0 < p.Lq) {
-            n = p.nb;
+        if (r0 < sq.Lq) {
+            n = sq.nb;
             if (p.causal) {
-                long long kmax = r0 + (BM - 1) + (p.Lk - p.Lq);
-                if (kmax > p.Lk - 1) kmax = p.Lk - 1;
+                long long kmax = r0 + (BM - 1) + (sq.Lk - sq.Lq);
+                if (kmax > sq.Lk - 1) kmax = sq.Lk - 1;
                 n = kmax < 0 ? 0 : (int)(kmax / C::BN) + 1;
             }
         }
@@ -330,16 +349,18 @@ attn_prefill64_kernel(const __grid_constant__ CUtensorMap mapQ, const __grid_con
                 const int blk = (p.kv_order == 0) ? it : n_it - 1 - it;
                 const int st = it % C::NS;
                 const uint32_t ph = (it / C::NS) & 1;
+                int kv_row, kv_slab;                         // (paged cache: one block-table entry per block)
+                kv_coords(p, b, h / (p.Hq / p.Hkv), kvh, blk, C::BN, kv_row, kv_slab);
                 ptx::mbar_wait(k_empty + st, ph ^ 1);
                 ptx::mbar_arrive_expect_tx(k_full + st, C::TILE);
                 for (int c = 0; c < C::NCH; ++c)
                     ptx::tma_load_3d(sK + st * C::TILE + c * (C::BN * 128), &mapK, k_full + st, c * C::CH,
-                                     blk * C::BN, kvh);
+                                     kv_row, kv_slab);
                 ptx::mbar_wait(v_empty + st, ph ^ 1);
                 ptx::mbar_arrive_expect_tx(v_full + st, C::TILE);
                 for (int c = 0; c < C::NCH; ++c)
                     ptx::tma_load_3d(sV + st * C::TILE + c * (C::BN * 128), &mapV, v_full + st, c * C::CH,
-                                     blk * C::BN, kvh);
+                                     kv_row, kv_slab);
             }
         }
     } else if (n_tile[warp - 16] > 0) {

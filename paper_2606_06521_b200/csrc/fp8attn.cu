@@ -517,7 +517,6 @@ int fp8attn_fwd(const void* q, const void* k, const void* v, void* o, int B, int
     p.block_table = paged ? stats->block_table : nullptr;
     p.page_size = paged ? stats->page_size : 0;
     p.max_pages = paged ? stats->max_pages : 0;
-    const bool varlen = p.seqlens_q || p.seqlens_k || paged;
     p.num_splits = ns;
     p.nb = nb;
     p.q_slabs = (int)q_slabs;
@@ -539,9 +538,8 @@ int fp8attn_fwd(const void* q, const void* k, const void* v, void* o, int B, int
     // modes 1 and 2 (Bn = 128 and Bn = 64); the decode kernel serves decode shapes with any split count; each
     // has a statistics instance (same schedule + P dump + underflow counters).  Everything else -- FP32
     // inputs, the no-cast mode, d = 64, prefill with splits -- runs on the general kernel.
-    // (not built into the prefill kernels: the sink-blocks-last order; the dynamic scale with Bn = 64)
-    const bool prefill_ok = d == 128 && ns == 1 && npl == 1 && pm != 0 && dt != 3 && kv_order != FP8ATTN_ORDER_SINK_LAST &&
-                            !(dynamic && bn == 64) && !(varlen && bn == 64);
+    // (not built into the prefill kernels: the sink-blocks-last order)
+    const bool prefill_ok = d == 128 && ns == 1 && npl == 1 && pm != 0 && dt != 3 && kv_order != FP8ATTN_ORDER_SINK_LAST;
     if (want_kernel == 2 && !prefill_ok) return FP8ATTN_E_UNSUPPORTED;
     // (automatic selection keeps prefill-shaped calls that ask for the P dump or the underflow counters on the
     // general kernel, whose serial schedule is the reference for them; stats->kernel = 2 takes the statistics

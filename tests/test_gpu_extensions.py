@@ -34,6 +34,8 @@ def _compare(case, r, ref, refc, mode, bn, label, dynamic, rows_codes=None, uf_e
     ("bf16", 1, 2, 128, (1, 2, 1, 600, 1000, 128, False)),        # prefill kernel (max warps carry the exponent)
     ("e4m3", 2, 2, 128, (1, 2, 2, 384, 1700, 128, True)),
     ("e4m3", 2, 2, 128, (1, 1, 1, 1280, 1280, 128, True)),
+    ("e4m3", 2, 2, 64, (1, 2, 2, 384, 1700, 128, True)),          # Bn = 64 prefill kernel: the exponent travels with the max
+    ("bf16", 1, 2, 64, (1, 2, 1, 600, 1000, 128, False)),
 ])
 @pytest.mark.parametrize("order", [0, 1])
 def test_dynamic_scale_matches_oracle(kind, mode, kernel, bn, shape, order):

@@ -92,10 +92,10 @@ def check_batches(r, per_batch, lens_q, Hq, Lq, causal, S, order, mode, bounds_o
 
 
 @pytest.mark.parametrize("kind,mode", [("e4m3", 2), ("bf16", 1)])
-@pytest.mark.parametrize("kernel", [1, 2])
+@pytest.mark.parametrize("kernel,bn", [(1, 128), (2, 128), (2, 64)])
 @pytest.mark.parametrize("paged", [False, True])
 @pytest.mark.parametrize("order", [0, 1])
-def test_varlen_paged_prefill(kind, mode, kernel, paged, order):
+def test_varlen_paged_prefill(kind, mode, kernel, bn, paged, order):
     B, Hq, Hkv, Lq = 3, 4, 2, 300
     lens_q, lens_k = [300, 77, 130], [1000, 517, 130]
     tq, tk, tv, sc, table, per_batch = build(kind, B, Hq, Hkv, Lq, lens_q, lens_k, 256, seed=31, paged=paged)
@@ -104,9 +104,10 @@ def test_varlen_paged_prefill(kind, mode, kernel, paged, order):
               seqlens_k=torch.tensor(lens_k, dtype=torch.int32, device=P.dev()))
     if paged:
         kw.update(block_table=table, Lk=max(lens_k))
-    r = f.fwd(tq, tk, tv, causal=True, S=256.0, kv_order=order, mode=mode, kernel=kernel, want_stats=True, **sc, **kw)
+    r = f.fwd(tq, tk, tv, causal=True, S=256.0, kv_order=order, mode=mode, kernel=kernel, block_n=bn, want_stats=True,
+              **sc, **kw)
     torch.cuda.synchronize()
-    assert r.kernel_id == kernel and r.block_n == 128
+    assert r.kernel_id == kernel and r.block_n == bn
     us, uo = check_batches(r, per_batch, lens_q, Hq, Lq, True, 256.0, order, mode)
     uf = r.underflow.cpu().numpy()
     slack = max(4, int(2e-3 * sum(lq * lk for lq, lk in zip(lens_q, lens_k)) * Hq))
