@@ -54,7 +54,9 @@ struct RowStat {
 };
 
 // ---- max warp (t, wq): Alg. 1 lines 4-6 for rows 32 wq .. 32 wq + 31 of tile t, then O <- alpha O ----
-template <int EB, bool FOLD>
+// EXT: the instance that carries the extensions (dynamic P scale, variable-length sequences, paged KV); the plain
+// instance has none of that code (measured: 1.3 % of cfg3).
+template <int EB, bool FOLD, bool EXT>
 __device__ __forceinline__ void prefill_max_warp(const FwdParams& p, int t, int wq, int lane, uint32_t tbase,
                                                  uint64_t* s_full_t, uint64_t* m_full_w, RowStat* mstat_t,
                                                  float* lscale_t, uint64_t* o_ready_t, int n_t, int row0, int bh, int kvh) {
@@ -62,13 +64,13 @@ __device__ __forceinline__ void prefill_max_warp(const FwdParams& p, int t, int 
     const uint32_t tlane = tbase + (static_cast<uint32_t>(wq * 32) << 16);
     const uint32_t tS = tlane + C::TM_S + t * 128, tO = tlane + C::TM_O + t * 128;
     const int rl = wq * 32 + lane;
-    const Seq sq = seq_of(p, bh / p.Hq, 128);
+    const Seq sq = EXT ? seq_of(p, bh / p.Hq, 128) : Seq{p.Lq, p.Lk, p.nb};
     const int jlim = last_visible_key(p, sq, row0 + rl);
     const int mask_from = mask_threshold(p, sq, row0, wq);
     float c_nat = p.sm_scale;
     if constexpr (EB == 1) c_nat *= p.q_scale[bh] * p.k_scale[kvh];
     const float cl2 = c_nat * LOG2E;
-    const bool dynamic = p.scale_mode == 1;         // reading R26 (the host launches the FOLD instance for it)
+    const bool dynamic = EXT && p.scale_mode == 1;  // reading R26 (the host launches the FOLD instance for it)
     const float log2S = (FOLD && !dynamic) ? log2f(p.S) : 0.0f;   // exact for S = 2^k
     float m_run = -INFINITY;
     int k_run = 0;            // dynamic: the exponent O and the row sums carry
@@ -155,11 +157,11 @@ __device__ __forceinline__ void prefill_max_warp(const FwdParams& p, int t, int 
 template <int EB, bool FOLD, int NPOLY, bool AUX>
 __device__ __forceinline__ void p_quarter(const uint32_t* v, uint32_t tS, int quarter, int j0, int jlim, uint64_t cl2_2,
                                           uint64_t negm_2, uint64_t s_2, uint64_t& sum_a, uint64_t& sum_b, uint64_t* bar,
-                                          int lane, uint8_t* dump_row, uint32_t* uf, const FwdParams& p) {
+                                          int lane, uint8_t* dump_row, uint32_t* uf, const FwdParams& p, bool sink_blk) {
     using C = PrefillCfg<EB>;
     uint32_t w[C::P_COLS / 4];
     exp_chunk<EB, FOLD, false, NPOLY>(v, w, j0 + quarter * 32, jlim, cl2_2, negm_2, s_2, sum_a, sum_b);
-    if constexpr (AUX) chunk_statistics<EB>(w, j0 + quarter * 32, jlim, dump_row, uf, p);
+    if constexpr (AUX) chunk_statistics<EB>(w, j0 + quarter * 32, jlim, dump_row, uf, p, sink_blk);
     if constexpr (EB == 1) ptx::tmem_st_x8(tS + quarter * 32, w);
     else ptx::tmem_st_x16(tS + quarter * 32, w);
     ptx::tmem_wait_st();
@@ -169,7 +171,7 @@ __device__ __forceinline__ void p_quarter(const uint32_t* v, uint32_t tS, int qu
 }
 
 // ---- exp warp (wq, half): Alg. 1 lines 7-9 and 12 for its rows of both tiles, its 64 key columns ----
-template <int EB, bool FOLD, bool AUX>
+template <int EB, bool FOLD, bool AUX, bool EXT>
 __device__ __forceinline__ void prefill_exp_warp(const FwdParams& p, int wq, int half, int lane, uint32_t tbase,
                                                  uint64_t* m_full, uint64_t* p_full, const RowStat* mstat, float* lsum,
                                                  const float* lscale,
@@ -188,8 +190,9 @@ __device__ __forceinline__ void prefill_exp_warp(const FwdParams& p, int wq, int
     const float cl2 = c_nat * LOG2E;
     const uint64_t cl2_2 = ptx::pack2(cl2, cl2), s_2 = ptx::pack2(p.S, p.S);
 
-    const Seq sq = seq_of(p, bh / p.Hq, 128);
+    const Seq sq = EXT ? seq_of(p, bh / p.Hq, 128) : Seq{p.Lq, p.Lk, p.nb};
     int jlim[2], first[2], mask_from[2];
+    bool count_row[2];        // AUX: this row exists and its zero codes are counted
     uint8_t* dump_row[2];     // AUX: this row of the P dump (fp8attn_stats.p_codes), else null
     uint32_t uf_sink = 0, uf_other = 0;   // AUX: zero codes among visible non-sink keys (sink block / other blocks)
     float l_run[2] = {0.0f, 0.0f};
@@ -199,6 +202,7 @@ __device__ __forceinline__ void prefill_exp_warp(const FwdParams& p, int wq, int
         jlim[t] = last_visible_key(p, sq, row0 + rl);
         mask_from[t] = mask_threshold(p, sq, row0, wq);
         first[t] = (p.kv_order == 0) ? 0 : n_it - n_tile[t];
+        count_row[t] = AUX && p.underflow != nullptr && row0 + rl < sq.Lq;
         dump_row[t] = (AUX && p.p_codes != nullptr && bh == p.p_bh && row0 + rl < sq.Lq)
                           ? p.p_codes + (size_t)(row0 + rl) * p.Lk
                           : nullptr;
@@ -247,17 +251,18 @@ __device__ __forceinline__ void prefill_exp_warp(const FwdParams& p, int wq, int
             // l = 0 in the epilogue)
             // AUX: the counter this block adds to (blocks that hold a sink key / all others); rows >= Lq do not
             // exist and are not counted
-            uint32_t* const uf = (AUX && p.underflow != nullptr && (pair * 2 + t) * BM + rl < sq.Lq)
-                                     ? (sink_in_range(p, j0, 128) ? &uf_sink : &uf_other)
+            const bool sink_blk = AUX && sink_in_range(p, j0, 128);
+            uint32_t* const uf = (AUX && count_row[t])
+                                     ? (sink_blk ? &uf_sink : &uf_other)
                                      : nullptr;
             p_quarter<EB, FOLD, CK::NPOLY, AUX>(r, tS, 2 * half, j0, jlim[t], cl2_2, negm_2, s_2, sum_a, sum_b,
-                                                p_full + 2 * t + 0, lane, dump_row[t], uf, p);
+                                                p_full + 2 * t + 0, lane, dump_row[t], uf, p, sink_blk);
             if (probe_next) {
                 ptx::mbar_probe(m_full + 4 * (t ^ 1) + wq, c_o & 1);
                 probed_tile = t ^ 1;
             }
             p_quarter<EB, FOLD, CK::NPOLY, AUX>(r + 32, tS, 2 * half + 1, j0, jlim[t], cl2_2, negm_2, s_2, sum_a,
-                                                sum_b, p_full + 2 * t + 1, lane, dump_row[t], uf, p);
+                                                sum_b, p_full + 2 * t + 1, lane, dump_row[t], uf, p, sink_blk);
             float sa, sb, sc, sd;
             ptx::unpack2(sum_a, sa, sb);
             ptx::unpack2(sum_b, sc, sd);
@@ -349,7 +354,7 @@ __device__ __forceinline__ void prefill_exp_warp(const FwdParams& p, int wq, int
 }
 // ---- the kernel ---------------------------------------------------------------------------------
 // grid = ceil(Lq / 256) * B*Hq CTAs in one dimension (order: see below).
-template <int EB, bool FOLD, bool AUX = false>
+template <int EB, bool FOLD, bool AUX = false, bool EXT = false>
 __global__ void __launch_bounds__(640, 1)
 attn_prefill_kernel(const __grid_constant__ CUtensorMap mapQ, const __grid_constant__ CUtensorMap mapK,
                      const __grid_constant__ CUtensorMap mapV, const __grid_constant__ CUtensorMap mapO,
@@ -393,7 +398,7 @@ attn_prefill_kernel(const __grid_constant__ CUtensorMap mapQ, const __grid_const
     const int kvh = b * p.Hkv + h / (p.Hq / p.Hkv);
 
     // visible block count of each tile (bottom-right causal, reading R15; this batch element's lengths)
-    const Seq sq = seq_of(p, b, C::BN);
+    const Seq sq = EXT ? seq_of(p, b, C::BN) : Seq{p.Lq, p.Lk, p.nb};
     int n_tile[2];
 #pragma unroll
     for (int t = 0; t < 2; ++t) {
@@ -443,12 +448,12 @@ attn_prefill_kernel(const __grid_constant__ CUtensorMap mapQ, const __grid_const
 
     if (warp < 8) {
         ptx::setmaxnreg_inc<C4::REG_EXP>();
-        prefill_exp_warp<EB, FOLD, AUX>(p, warp & 3, warp >> 2, lane, tbase, m_full, p_full, mstat, lsum, lscale, o_done, n_tile,
+        prefill_exp_warp<EB, FOLD, AUX, EXT>(p, warp & 3, warp >> 2, lane, tbase, m_full, p_full, mstat, lsum, lscale, o_done, n_tile,
                                         n_it, pair, bh, kvh, &mapO, sK, sV);
     } else if (warp < 16) {
         ptx::setmaxnreg_dec<C4::REG_MAX>();
         const int t = (warp - 8) >> 2, wq = warp & 3;
-        prefill_max_warp<EB, FOLD>(p, t, wq, lane, tbase, s_full + t, m_full + 4 * t + wq, mstat + t * 2 * 128,
+        prefill_max_warp<EB, FOLD, EXT>(p, t, wq, lane, tbase, s_full + t, m_full + 4 * t + wq, mstat + t * 2 * 128,
                                    lscale + t * 128, o_ready + t, n_tile[t], (pair * 2 + t) * BM, bh, kvh);
     } else {
         ptx::setmaxnreg_dec<C4::REG_MISC>();
@@ -466,8 +471,8 @@ attn_prefill_kernel(const __grid_constant__ CUtensorMap mapQ, const __grid_const
                     const int blk = (p.kv_order == 0) ? it : n_it - 1 - it;
                     const int st = it % C::NS;
                     const uint32_t ph = (it / C::NS) & 1;
-                    int kv_row, kv_slab;                     // (paged cache: one block-table entry per block)
-                    kv_coords(p, b, h / (p.Hq / p.Hkv), kvh, blk, C::BN, kv_row, kv_slab);
+                    int kv_row = blk * C::BN, kv_slab = kvh;
+                    if constexpr (EXT) kv_coords(p, b, h / (p.Hq / p.Hkv), kvh, blk, C::BN, kv_row, kv_slab);   // paged cache
                     ptx::mbar_wait(k_empty + st, ph ^ 1);
                     ptx::mbar_arrive_expect_tx(k_full + st, C::TILE);
                     for (int c = 0; c < C::NCH; ++c)

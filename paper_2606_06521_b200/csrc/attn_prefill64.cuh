@@ -92,6 +92,7 @@ __device__ __forceinline__ void prefill64_softmax(const FwdParams& p, int t, int
         const int blk = (p.kv_order == 0) ? c : n_t - 1 - c;
         const int j0 = blk * C::BN;
         const bool mask = (j0 + C::BN - 1 > warp_vis) || (j0 + C::BN > sq.Lk);
+        const bool sink_blk = AUX && sink_in_range(p, j0, C::BN);
         ptx::mbar_wait(s_full + par, (c >> 1) & 1);
         ptx::tc_fence_after();
         // ---- lines 4-5: block max, running max ----
@@ -153,8 +154,8 @@ __device__ __forceinline__ void prefill64_softmax(const FwdParams& p, int t, int
             if (mask) exp_chunk<EB, FOLD, true>(v, w, j0 + cb * 32, jlim, cl2_2, negm_2, s_2, sum_a, sum_b);
             else exp_chunk<EB, FOLD, false>(v, w, j0 + cb * 32, jlim, cl2_2, negm_2, s_2, sum_a, sum_b);
             if constexpr (AUX)
-                chunk_statistics<EB>(w, j0 + cb * 32, jlim, dump_row,
-                                     count ? (sink_in_range(p, j0, C::BN) ? &uf_sink : &uf_other) : nullptr, p);
+                chunk_statistics<EB>(w, j0 + cb * 32, jlim, dump_row, count ? (sink_blk ? &uf_sink : &uf_other) : nullptr, p,
+                                     sink_blk);
             // (P of chunk cb lands on columns of chunk 0, whose logits are already in registers)
             if constexpr (EB == 1) ptx::tmem_st_x8(tS + cb * 8, w);
             else ptx::tmem_st_x16(tS + cb * 16, w);

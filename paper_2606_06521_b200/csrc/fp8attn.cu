@@ -228,13 +228,21 @@ int launch_prefill(const CUtensorMap& mq, const CUtensorMap& mk, const CUtensorM
     CUtensorMap mo;
     if (int rc = make_map(&mo, p.o, p.o_bf16 ? 2 : 4, (long long)p.B * p.Hq, p.Lq, 128, 32)) return rc;
     const dim3 grid((unsigned)(((p.Lq + 2 * BM - 1) / (2 * BM)) * (p.B * p.Hq)));
+    // the extensions (dynamic scale, variable-length sequences, paged KV) live in their own instance, like the
+    // statistics: the plain instance is the headline path and carries no code it does not need
+    const bool ext = p.scale_mode == 1 || p.seqlens_q || p.seqlens_k || p.block_table;
     if (aux) {
-        auto kern = attn_prefill_kernel<EB, FOLD, true>;
+        auto kern = attn_prefill_kernel<EB, FOLD, true, true>;
+        static std::atomic<unsigned long long> done{0};
+        if (int rc = ensure_smem(kern, C::SMEM_BYTES, done)) return rc;
+        kern<<<grid, C::THREADS, C::SMEM_BYTES, st>>>(mq, mk, mv, mo, p);
+    } else if (ext) {
+        auto kern = attn_prefill_kernel<EB, FOLD, false, true>;
         static std::atomic<unsigned long long> done{0};
         if (int rc = ensure_smem(kern, C::SMEM_BYTES, done)) return rc;
         kern<<<grid, C::THREADS, C::SMEM_BYTES, st>>>(mq, mk, mv, mo, p);
     } else {
-        auto kern = attn_prefill_kernel<EB, FOLD, false>;
+        auto kern = attn_prefill_kernel<EB, FOLD, false, false>;
         static std::atomic<unsigned long long> done{0};
         if (int rc = ensure_smem(kern, C::SMEM_BYTES, done)) return rc;
         kern<<<grid, C::THREADS, C::SMEM_BYTES, st>>>(mq, mk, mv, mo, p);

@@ -132,10 +132,11 @@ __device__ __forceinline__ void mask32(uint32_t* v, int j_first, int jlim) {
 // exp_chunk leaves it; BF16 mode recovers a code from its exact BF16 value: times 2^-120, shifted right by 4.
 template <int EB>
 __device__ __forceinline__ void chunk_statistics(const uint32_t* w, int jq, int jlim, uint8_t* dump_row, uint32_t* uf,
-                                                 const FwdParams& p) {
+                                                 const FwdParams& p, bool sink_blk) {
     constexpr int NW = 8 * EB;      // words of the chunk
     if (dump_row == nullptr && uf == nullptr) return;
-    const uint32_t sinks = sink_mask32(p, jq);        // which keys of the chunk are sink keys
+    // which keys of the chunk are sink keys (sink_blk: the KV block of the chunk holds one at all)
+    const uint32_t sinks = sink_blk ? sink_mask32(p, jq) : 0u;
     if (dump_row == nullptr && sinks == 0u && jq + 31 <= jlim) {
         // every key of the chunk is visible and none is a sink: count the zero codes a word at a time
         uint32_t zeros = 0;
