@@ -54,12 +54,84 @@ struct RowStat {
 };
 
 // ---- max warp (t, wq): Alg. 1 lines 4-6 for rows 32 wq .. 32 wq + 31 of tile t, then O <- alpha O ----
+// ---- line 12 for one (tile, column half): O / (S l) of 32 rows x 64 columns, written as 32-row x 128-byte boxes
+// (128-byte swizzle; FP32: two boxes of 32 floats, BF16: one box of 64) into the K / V ring -- no MMA reads it any
+// more once both tiles are done -- and stored with TMA (rows >= Lq are clipped by the map).  The four warps that can
+// read a 32-lane quarter of TMEM (two exp warps, the max warps of both tiles) take one (tile, half) each.
+template <int EB, bool FOLD>
+__device__ __forceinline__ void prefill_store_half(const FwdParams& p, int t, int half, int wq, int lane, uint32_t tbase,
+                                                   const float* lsum, const float* lscale, uint64_t* o_done, bool has_blocks,
+                                                   bool other_has_blocks,
+                                                   int row0, int bh, float vs, const CUtensorMap* mapO, uint8_t* stage,
+                                                   bool write_row_sum) {
+    using C = PrefillCfg<EB>;
+    const int rl = wq * 32 + lane;
+    // both tiles must be done: the staging area is the K / V ring, which the other tile's MMAs may still read
+    if (has_blocks) ptx::mbar_wait(o_done + t, 0);
+    if (other_has_blocks) ptx::mbar_wait(o_done + (t ^ 1), 0);
+    ptx::tc_fence_after();
+    const float l_all = lsum[(t * 2) * 128 + rl] + lsum[(t * 2 + 1) * 128 + rl];
+    // l_all and O carry the same factor: S when the static scale is folded into the exponent, the last block's 2^k
+    // under the dynamic scale (published by the max warp), 1 otherwise
+    const float carried = has_blocks ? lscale[t * 128 + rl] : 1.0f;
+    if (write_row_sum && row0 + rl < p.Lq && p.row_sum != nullptr) p.row_sum[(long long)bh * p.Lq + row0 + rl] = l_all / carried;
+    const float inv = (l_all > 0.0f) ? (FOLD ? vs / l_all : vs / (p.S * l_all)) : 0.0f;
+    if (row0 >= p.Lq) return;                   // no row of this tile exists (warp-uniform)
+    const uint32_t tO = tbase + (static_cast<uint32_t>(wq * 32) << 16) + C::TM_O + t * 128 + half * 64;
+#pragma unroll 1
+    for (int cb = 0; cb < 2; ++cb) {
+        const int ch = half * 2 + cb;           // 32-column chunk of the output row
+        uint32_t v[32];
+        if (has_blocks) {
+            ptx::tmem_ld_x32(tO + cb * 32, v);
+            ptx::tmem_wait_ld();
+        } else {
+#pragma unroll
+            for (int e = 0; e < 32; ++e) v[e] = 0u;
+        }
+        if (p.o_bf16) {
+            uint8_t* box = stage + (half * 8 + wq) * 4096;
+#pragma unroll
+            for (int j = 0; j < 4; ++j) {
+                uint4 w4;
+                w4.x = ptx::cvt_bf16x2(__uint_as_float(v[8 * j]) * inv, __uint_as_float(v[8 * j + 1]) * inv);
+                w4.y = ptx::cvt_bf16x2(__uint_as_float(v[8 * j + 2]) * inv, __uint_as_float(v[8 * j + 3]) * inv);
+                w4.z = ptx::cvt_bf16x2(__uint_as_float(v[8 * j + 4]) * inv, __uint_as_float(v[8 * j + 5]) * inv);
+                w4.w = ptx::cvt_bf16x2(__uint_as_float(v[8 * j + 6]) * inv, __uint_as_float(v[8 * j + 7]) * inv);
+                *reinterpret_cast<uint4*>(box + lane * 128 + (((cb * 4 + j) ^ (lane & 7)) << 4)) = w4;
+            }
+            if (cb == 1) {
+                ptx::fence_proxy_async_smem();
+                __syncwarp();
+                if (lane == 0) ptx::tma_store_3d(mapO, box, half * 64, row0 + wq * 32, bh);
+            }
+            continue;
+        }
+        uint8_t* box = stage + (ch * 4 + wq) * 4096;
+#pragma unroll
+        for (int j = 0; j < 8; ++j) {
+            const float4 o4 = make_float4(__uint_as_float(v[4 * j]) * inv, __uint_as_float(v[4 * j + 1]) * inv,
+                                          __uint_as_float(v[4 * j + 2]) * inv, __uint_as_float(v[4 * j + 3]) * inv);
+            *reinterpret_cast<float4*>(box + lane * 128 + ((j ^ (lane & 7)) << 4)) = o4;
+        }
+        ptx::fence_proxy_async_smem();
+        __syncwarp();
+        if (lane == 0) ptx::tma_store_3d(mapO, box, ch * 32, row0 + wq * 32, bh);
+    }
+    if (lane == 0) {
+        ptx::bulk_commit_group();
+        ptx::bulk_wait_group_read0();
+    }
+}
+
 // EXT: the instance that carries the extensions (dynamic P scale, variable-length sequences, paged KV); the plain
 // instance has none of that code (measured: 1.3 % of cfg3).
 template <int EB, bool FOLD, bool EXT>
 __device__ __forceinline__ void prefill_max_warp(const FwdParams& p, int t, int wq, int lane, uint32_t tbase,
                                                  uint64_t* s_full_t, uint64_t* m_full_w, RowStat* mstat_t,
-                                                 float* lscale_t, uint64_t* o_ready_t, int n_t, int row0, int bh, int kvh) {
+                                                 float* lscale_t, uint64_t* o_ready_t, int n_t, int row0, int bh, int kvh,
+                                                 const float* lsum, uint64_t* o_done, int n_other, const CUtensorMap* mapO,
+                                                 uint8_t* stage) {
     using C = PrefillCfg<EB>;
     const uint32_t tlane = tbase + (static_cast<uint32_t>(wq * 32) << 16);
     const uint32_t tS = tlane + C::TM_S + t * 128, tO = tlane + C::TM_O + t * 128;
@@ -150,6 +222,12 @@ __device__ __forceinline__ void prefill_max_warp(const FwdParams& p, int t, int 
     const int qrow = row0 + rl;
     if (p.row_max != nullptr && qrow < p.Lq)
         p.row_max[(long long)bh * p.Lq + qrow] = (m_run == -INFINITY) ? -INFINITY : m_run * c_nat;
+    // this warp's share of the epilogue: (tile t, the column half the exp warps do not store)
+    float vs = 1.0f;
+    if constexpr (EB == 1) vs = p.v_scale[kvh];
+    ptx::named_bar_sync(1 + wq, 128);           // the row sums of the exp warps are in shared memory
+    prefill_store_half<EB, FOLD>(p, t, 1 - t, wq, lane, tbase, lsum, lscale_t - t * 128, o_done, n_t > 0, n_other > 0, row0,
+                                 bh, vs, mapO, stage, false);
 }
 
 // One P quarter: exp / sum / cast (exp_chunk), statistics (AUX), P over the head of its S quarter in TMEM (the A
@@ -280,77 +358,18 @@ __device__ __forceinline__ void prefill_exp_warp(const FwdParams& p, int wq, int
         }
     }
     // ---- line 12: O / (S l), row sum.  The two warps of a row add their partial sums (same running max, so they
-    // just add).  Each warp owns 32 rows x 64 output columns of each tile: it scales them, writes them as two
-    // 32-row x 128-byte boxes (128-byte swizzle) into the K / V ring, which no MMA reads any more once both tiles
-    // are done, and stores the boxes with TMA (rows >= Lq are clipped by the map) ----
+    // just add); then this warp stores (tile `half`, column half `half`), see prefill_store_half ----
 #pragma unroll
     for (int t = 0; t < 2; ++t)
         lsum[(t * 2 + half) * 128 + rl] = (jlim[t] < 0) ? 0.0f : l_run[t];     // no visible key: l = 0 exactly
-    ptx::named_bar_sync(1 + wq, 64);            // the two warps that share these rows
-#pragma unroll
-    for (int t = 0; t < 2; ++t) {
-        if (n_tile[t] > 0) ptx::mbar_wait(o_done + t, 0);
+    ptx::named_bar_sync(1 + wq, 128);           // the four warps of this 32-row group (2 exp + 2 max)
+    if (half == 0 && p.row_sum != nullptr) {    // the row sum of the tile this warp does not store
+        const int row1 = (pair * 2 + 1) * BM + rl;
+        const float l1 = lsum[2 * 128 + rl] + lsum[3 * 128 + rl];
+        if (row1 < p.Lq) p.row_sum[(long long)bh * p.Lq + row1] = l1 / ((n_tile[1] > 0) ? lscale[128 + rl] : 1.0f);
     }
-    ptx::tc_fence_after();
-#pragma unroll
-    for (int t = 0; t < 2; ++t) {
-        const int row0 = (pair * 2 + t) * BM;
-        const int qrow = row0 + rl;
-        const float l_all = lsum[(t * 2) * 128 + rl] + lsum[(t * 2 + 1) * 128 + rl];
-        // l_all and O carry the same factor: S when the static scale is folded into the exponent, the last
-        // block's 2^k under the dynamic scale (published by the max warp), 1 otherwise
-        const float carried = (n_tile[t] > 0) ? lscale[t * 128 + rl] : 1.0f;
-        if (qrow < p.Lq && half == 0 && p.row_sum != nullptr) p.row_sum[(long long)bh * p.Lq + qrow] = l_all / carried;
-        const float inv = (l_all > 0.0f) ? (FOLD ? vs / l_all : vs / (p.S * l_all)) : 0.0f;
-        if (row0 >= p.Lq) continue;             // no row of this tile exists (warp-uniform)
-        const uint32_t tO = tlane + C::TM_O + t * 128 + half * 64;
-        uint8_t* stage = t ? stage1 : stage0;
-#pragma unroll 1
-        for (int cb = 0; cb < 2; ++cb) {
-            const int ch = half * 2 + cb;       // 32-column chunk of the output row
-            uint32_t v[32];
-            if (n_tile[t] > 0) {
-                ptx::tmem_ld_x32(tO + cb * 32, v);
-                ptx::tmem_wait_ld();
-            } else {
-#pragma unroll
-                for (int e = 0; e < 32; ++e) v[e] = 0u;
-            }
-            if (p.o_bf16) {
-                // one 32-row x 64-column BF16 box (128-byte rows) per warp and tile: chunk cb fills half of it
-                uint8_t* box = stage + (half * 8 + wq) * 4096;
-#pragma unroll
-                for (int j = 0; j < 4; ++j) {
-                    uint4 w4;
-                    w4.x = ptx::cvt_bf16x2(__uint_as_float(v[8 * j]) * inv, __uint_as_float(v[8 * j + 1]) * inv);
-                    w4.y = ptx::cvt_bf16x2(__uint_as_float(v[8 * j + 2]) * inv, __uint_as_float(v[8 * j + 3]) * inv);
-                    w4.z = ptx::cvt_bf16x2(__uint_as_float(v[8 * j + 4]) * inv, __uint_as_float(v[8 * j + 5]) * inv);
-                    w4.w = ptx::cvt_bf16x2(__uint_as_float(v[8 * j + 6]) * inv, __uint_as_float(v[8 * j + 7]) * inv);
-                    *reinterpret_cast<uint4*>(box + lane * 128 + (((cb * 4 + j) ^ (lane & 7)) << 4)) = w4;
-                }
-                if (cb == 1) {
-                    ptx::fence_proxy_async_smem();
-                    __syncwarp();
-                    if (lane == 0) ptx::tma_store_3d(mapO, box, half * 64, row0 + wq * 32, bh);
-                }
-                continue;
-            }
-            uint8_t* box = stage + (ch * 4 + wq) * 4096;
-#pragma unroll
-            for (int j = 0; j < 8; ++j) {
-                const float4 o4 = make_float4(__uint_as_float(v[4 * j]) * inv, __uint_as_float(v[4 * j + 1]) * inv,
-                                              __uint_as_float(v[4 * j + 2]) * inv, __uint_as_float(v[4 * j + 3]) * inv);
-                *reinterpret_cast<float4*>(box + lane * 128 + ((j ^ (lane & 7)) << 4)) = o4;
-            }
-            ptx::fence_proxy_async_smem();
-            __syncwarp();
-            if (lane == 0) ptx::tma_store_3d(mapO, box, ch * 32, row0 + wq * 32, bh);
-        }
-    }
-    if (lane == 0) {
-        ptx::bulk_commit_group();
-        ptx::bulk_wait_group_read0();
-    }
+    prefill_store_half<EB, FOLD>(p, half, half, wq, lane, tbase, lsum, lscale, o_done, n_tile[half] > 0,
+                                 n_tile[half ^ 1] > 0, (pair * 2 + half) * BM, bh, vs, mapO, half ? stage1 : stage0, half == 0);
 }
 // ---- the kernel ---------------------------------------------------------------------------------
 // grid = ceil(Lq / 256) * B*Hq CTAs in one dimension (order: see below).
@@ -454,7 +473,8 @@ attn_prefill_kernel(const __grid_constant__ CUtensorMap mapQ, const __grid_const
         ptx::setmaxnreg_dec<C4::REG_MAX>();
         const int t = (warp - 8) >> 2, wq = warp & 3;
         prefill_max_warp<EB, FOLD, EXT>(p, t, wq, lane, tbase, s_full + t, m_full + 4 * t + wq, mstat + t * 2 * 128,
-                                   lscale + t * 128, o_ready + t, n_tile[t], (pair * 2 + t) * BM, bh, kvh);
+                                   lscale + t * 128, o_ready + t, n_tile[t], (pair * 2 + t) * BM, bh, kvh, lsum, o_done,
+                                   n_tile[t ^ 1], &mapO, t ? sV : sK);
     } else {
         ptx::setmaxnreg_dec<C4::REG_MISC>();
         if (warp == 18) {
