@@ -167,6 +167,19 @@ def test_cfg4_full_size_sampled_rows(kind, mode):
             del r
     # the paper's effect, on the GPU output: forward S=1 is the worst of the four
     assert mses[(1.0, 0)] > 1.2 * mses[(256.0, 1)]
+    # the P codes of that head at full size (64 sampled rows x up to 16384 keys) from the statistics instance of the
+    # same kernel, in the two configurations that differ most (forward S = 1 collapses, reverse S = 256 does not)
+    rows_c = rows_of_head(cfg.Lq, 64, seed=5)
+    for S, order in ((1.0, 0), (256.0, 1)):
+        rd = f.fwd(q, k, v, causal=True, S=S, kv_order=order, mode=mode, dump_head=(b, h), kernel=2, **sc)
+        torch.cuda.synchronize()
+        assert rd.kernel_id == 2
+        ref = oracle.attention_fwd(qo, ko, vo, causal=True, S=S, kv_order=order, mode=mode, in_dtype=dt,
+                                   block_n=rd.block_n, rows=rows_c, want_codes=True, **kw)
+        g = rd.p_codes[torch.from_numpy(rows_c).to(rd.p_codes.device)].cpu().numpy()
+        match, n_flip, _ = P.check_codes(g, ref.p_codes, mode, label=f"cfg4 {kind} S={S} order={order}")
+        print(f"cfg4 {kind} S={S} order={order}: P code match {match:.6f} over {int((ref.p_codes != 0xFF).sum())} elements")
+        del rd
 
 
 # ------------------------------------------------------------------ config 5 (decode)
