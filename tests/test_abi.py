@@ -91,3 +91,44 @@ def test_product_path_does_not_import_the_oracle():
         if f.endswith((".py", ".c")):
             src = open(os.path.join(orc, f)).read()
             assert not re.search(r"^\s*(from|import)\s+paper_2606_06521_b200\b", src, re.M), f
+
+
+def test_stats_struct_fields_follow_the_header(fa):
+    """The ctypes mirror of fp8attn_stats lists the header's fields in the header's order (a field added on one side
+    only would shift every later field)."""
+    text = open(HEADER).read()
+    body = text[text.index("typedef struct fp8attn_stats {") + len("typedef struct fp8attn_stats {"):text.index("} fp8attn_stats;")]
+    body = re.sub(r"/\*.*?\*/", "", body, flags=re.S)
+    names = []
+    for decl in body.split(";"):
+        decl = decl.strip()
+        if not decl or decl.startswith("typedef"):
+            continue
+        for part in decl.split(","):
+            m = re.search(r"(\w+)\s*(\[[^\]]*\])?\s*$", part.strip())
+            names.append(m.group(1))
+    assert names == [n for n, _ in fa.Stats._fields_], (names, [n for n, _ in fa.Stats._fields_])
+
+
+def test_new_options_are_validated_before_any_cuda_call(fa):
+    one = C.c_void_p(16)
+    st = fa.Stats()
+    st.struct_size = C.sizeof(fa.Stats)
+    call = lambda: fa.fp8attn_fwd(one, one, one, one, 1, 1, 1, 8, 8, 64, 0, 1.0, 0, 1 | fa.DTYPE_BF16, C.byref(st))
+    st.scale_mode = 2
+    assert call() == -4
+    st.scale_mode, st.o_dtype = 0, 3
+    assert call() == -4
+    st.o_dtype = 0
+    bad = (C.c_int32 * 2)(5, 3)                     # not ascending
+    st.sink_pos, st.n_sink = C.cast(bad, C.c_void_p), 2
+    assert call() == -2
+    ok = (C.c_int32 * 2)(3, 9)                      # past the last key
+    st.sink_pos = C.cast(ok, C.c_void_p)
+    assert call() == -2
+    st.sink_pos, st.n_sink = None, 4
+    st.block_table, st.page_size, st.max_pages, st.num_pages = 16, 4, 1, 1      # table does not reach Lk = 8
+    assert call() == -2
+    st.block_table = None
+    st.scale_mode = 1                               # the dynamic scale needs a cast: not in the no-cast mode
+    assert fa.fp8attn_fwd(one, one, one, one, 1, 1, 1, 8, 8, 64, 0, 1.0, 0, 0 | fa.DTYPE_BF16, C.byref(st)) == -4
