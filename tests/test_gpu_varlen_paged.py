@@ -146,3 +146,34 @@ def test_varlen_arguments():
     with pytest.raises(f.Fp8AttnError) as e:      # the table does not reach Lk
         f.fwd(tq, tk, tv, causal=True, S=256.0, kv_order=1, mode=2, block_table=table, Lk=1000, **sc)
     assert e.value.code == -2
+
+
+@pytest.mark.parametrize("kernel", [1, 2])
+def test_varlen_degenerate_lengths(kernel):
+    """Empty sequences, a sequence with more query rows than keys (rows that see nothing), and full-length ones in
+    the same call: the degenerate cases of the per-sequence geometry."""
+    B, Hq, Hkv, Lq = 4, 2, 1, 260
+    lens_q, lens_k = [0, 260, 200, 1], [300, 0, 120, 257]
+    lens_k_build = [max(1, x) for x in lens_k]          # the builder needs one key; seqlens_k still says 0
+    tq, tk, tv, sc, table, per_batch = build("e4m3", B, Hq, Hkv, Lq, [max(1, x) for x in lens_q], lens_k_build, 128,
+                                             seed=41, paged=False)
+    f = P.fa()
+    r = f.fwd(tq, tk, tv, causal=True, S=256.0, kv_order=1, mode=2, kernel=kernel, want_stats=True,
+              seqlens_q=torch.tensor(lens_q, dtype=torch.int32, device=P.dev()),
+              seqlens_k=torch.tensor(lens_k, dtype=torch.int32, device=P.dev()), **sc)
+    torch.cuda.synchronize()
+    assert r.kernel_id == kernel
+    o, rm, rs = r.o.cpu().numpy(), r.row_max.cpu().numpy(), r.row_sum.cpu().numpy()
+    assert np.all(np.isfinite(o))
+    for b in (0, 1):                                    # no query rows / no keys: nothing is computed
+        assert np.all(o[b] == 0) and np.all(np.isneginf(rm[b])) and np.all(rs[b] == 0)
+    # b = 2: 200 rows against 120 keys, bottom-right aligned: the first 80 rows see nothing
+    assert np.all(o[2, :, :80] == 0) and np.all(np.isneginf(rm[2, :, :80]))
+    for b in (2, 3):
+        qc, kc, vc, dt, kw = per_batch[b]
+        lq, lk = lens_q[b], lens_k[b]
+        ref = oracle.attention_fwd(qc[:, :, :lq], kc[:, :, :lk], vc[:, :, :lk], causal=True, S=256.0, kv_order=1, mode=2,
+                                   in_dtype=dt, block_n=r.block_n, **kw)
+        got = o[b, :, :lq].reshape(-1, 128).astype(np.float64)
+        assert P.rel_l2(got, ref.out) <= P.REL_L2[2]
+        assert np.all(o[b, :, lq:] == 0)
