@@ -235,17 +235,19 @@ __device__ __forceinline__ void prefill_max_warp(const FwdParams& p, int t, int 
 template <int EB, bool FOLD, int NPOLY, bool AUX>
 __device__ __forceinline__ void p_quarter(const uint32_t* v, uint32_t tS, int quarter, int j0, int jlim, uint64_t cl2_2,
                                           uint64_t negm_2, uint64_t s_2, uint64_t& sum_a, uint64_t& sum_b, uint64_t* bar,
-                                          int lane, uint8_t* dump_row, uint32_t* uf, const FwdParams& p, bool sink_blk) {
+                                          int lane, uint8_t* dump_row, bool count, uint32_t& zeros, const FwdParams& p,
+                                          bool sink_blk) {
     using C = PrefillCfg<EB>;
     uint32_t w[C::P_COLS / 4];
     exp_chunk<EB, FOLD, false, NPOLY>(v, w, j0 + quarter * 32, jlim, cl2_2, negm_2, s_2, sum_a, sum_b);
-    if constexpr (AUX) chunk_statistics<EB>(w, j0 + quarter * 32, jlim, dump_row, uf, p, sink_blk);
     if constexpr (EB == 1) ptx::tmem_st_x8(tS + quarter * 32, w);
     else ptx::tmem_st_x16(tS + quarter * 32, w);
     ptx::tmem_wait_st();
     ptx::tc_fence_before();
     __syncwarp();
     if (lane == 0) ptx::mbar_arrive(bar);
+    // (after the hand-off: the statistics are not on the path the tensor pipe waits for)
+    if constexpr (AUX) zeros += chunk_statistics<EB>(w, j0 + quarter * 32, jlim, dump_row, count, p, sink_blk);
 }
 
 // ---- exp warp (wq, half): Alg. 1 lines 7-9 and 12 for its rows of both tiles, its 64 key columns ----
@@ -330,17 +332,20 @@ __device__ __forceinline__ void prefill_exp_warp(const FwdParams& p, int wq, int
             // AUX: the counter this block adds to (blocks that hold a sink key / all others); rows >= Lq do not
             // exist and are not counted
             const bool sink_blk = AUX && sink_in_range(p, j0, 128);
-            uint32_t* const uf = (AUX && count_row[t])
-                                     ? (sink_blk ? &uf_sink : &uf_other)
-                                     : nullptr;
+            uint32_t zeros = 0;
             p_quarter<EB, FOLD, CK::NPOLY, AUX>(r, tS, 2 * half, j0, jlim[t], cl2_2, negm_2, s_2, sum_a, sum_b,
-                                                p_full + 2 * t + 0, lane, dump_row[t], uf, p, sink_blk);
+                                                p_full + 2 * t + 0, lane, dump_row[t], count_row[t], zeros, p, sink_blk);
             if (probe_next) {
                 ptx::mbar_probe(m_full + 4 * (t ^ 1) + wq, c_o & 1);
                 probed_tile = t ^ 1;
             }
             p_quarter<EB, FOLD, CK::NPOLY, AUX>(r + 32, tS, 2 * half + 1, j0, jlim[t], cl2_2, negm_2, s_2, sum_a,
-                                                sum_b, p_full + 2 * t + 1, lane, dump_row[t], uf, p, sink_blk);
+                                                sum_b, p_full + 2 * t + 1, lane, dump_row[t], count_row[t], zeros, p,
+                                                sink_blk);
+            if constexpr (AUX) {
+                if (sink_blk) uf_sink += zeros;
+                else uf_other += zeros;
+            }
             float sa, sb, sc, sd;
             ptx::unpack2(sum_a, sa, sb);
             ptx::unpack2(sum_b, sc, sd);

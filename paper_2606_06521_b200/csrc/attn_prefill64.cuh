@@ -153,9 +153,11 @@ __device__ __forceinline__ void prefill64_softmax(const FwdParams& p, int t, int
             ptx::tmem_wait_ld();
             if (mask) exp_chunk<EB, FOLD, true>(v, w, j0 + cb * 32, jlim, cl2_2, negm_2, s_2, sum_a, sum_b);
             else exp_chunk<EB, FOLD, false>(v, w, j0 + cb * 32, jlim, cl2_2, negm_2, s_2, sum_a, sum_b);
-            if constexpr (AUX)
-                chunk_statistics<EB>(w, j0 + cb * 32, jlim, dump_row, count ? (sink_blk ? &uf_sink : &uf_other) : nullptr, p,
-                                     sink_blk);
+            if constexpr (AUX) {
+                const uint32_t zeros = chunk_statistics<EB>(w, j0 + cb * 32, jlim, dump_row, count, p, sink_blk);
+                if (sink_blk) uf_sink += zeros;
+                else uf_other += zeros;
+            }
             // (P of chunk cb lands on columns of chunk 0, whose logits are already in registers)
             if constexpr (EB == 1) ptx::tmem_st_x8(tS + cb * 8, w);
             else ptx::tmem_st_x16(tS + cb * 16, w);

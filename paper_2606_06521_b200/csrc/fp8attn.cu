@@ -231,8 +231,13 @@ int launch_prefill(const CUtensorMap& mq, const CUtensorMap& mk, const CUtensorM
     // the extensions (dynamic scale, variable-length sequences, paged KV) live in their own instance, like the
     // statistics: the plain instance is the headline path and carries no code it does not need
     const bool ext = p.scale_mode == 1 || p.seqlens_q || p.seqlens_k || p.block_table;
-    if (aux) {
+    if (aux && ext) {
         auto kern = attn_prefill_kernel<EB, FOLD, true, true>;
+        static std::atomic<unsigned long long> done{0};
+        if (int rc = ensure_smem(kern, C::SMEM_BYTES, done)) return rc;
+        kern<<<grid, C::THREADS, C::SMEM_BYTES, st>>>(mq, mk, mv, mo, p);
+    } else if (aux) {
+        auto kern = attn_prefill_kernel<EB, FOLD, true, false>;
         static std::atomic<unsigned long long> done{0};
         if (int rc = ensure_smem(kern, C::SMEM_BYTES, done)) return rc;
         kern<<<grid, C::THREADS, C::SMEM_BYTES, st>>>(mq, mk, mv, mo, p);

@@ -128,40 +128,58 @@ __device__ __forceinline__ void mask32(uint32_t* v, int j_first, int jlim) {
 
 // Statistics of one 32-key chunk of P (statistics instances only): the E4M3 codes of the visible keys go to
 // dump_row (this query row of the P dump of fp8attn_stats, or null) and the zero codes among the visible
-// non-sink keys are counted into *uf (Prop. 1; null = not counted).  w holds the chunk as
-// exp_chunk leaves it; BF16 mode recovers a code from its exact BF16 value: times 2^-120, shifted right by 4.
+// non-sink keys are counted and returned (Prop. 1; `count` false = not counted, 0).  w holds the
+// chunk as exp_chunk leaves it; BF16 mode recovers a code from its exact BF16 value: times 2^-120, shifted right by 4.
+// The general case (a dump, a sink key in the chunk, a masked key) is a function call: it runs for a few chunks per
+// row, and inlined four times it doubles the size of the loop the exp warps live in.
 template <int EB>
-__device__ __forceinline__ void chunk_statistics(const uint32_t* w, int jq, int jlim, uint8_t* dump_row, uint32_t* uf,
-                                                 const FwdParams& p, bool sink_blk) {
-    constexpr int NW = 8 * EB;      // words of the chunk
-    if (dump_row == nullptr && uf == nullptr) return;
-    // which keys of the chunk are sink keys (sink_blk: the KV block of the chunk holds one at all)
-    const uint32_t sinks = sink_blk ? sink_mask32(p, jq) : 0u;
-    if (dump_row == nullptr && sinks == 0u && jq + 31 <= jlim) {
-        // every key of the chunk is visible and none is a sink: count the zero codes a word at a time
-        uint32_t zeros = 0;
-#pragma unroll
-        for (int i = 0; i < NW; ++i)
-            zeros += (EB == 1) ? (__popc(__vcmpeq4(w[i], 0u)) >> 3) : (__popc(__vcmpeq2(w[i], 0u)) >> 4);
-        *uf += zeros;
-        return;
-    }
+struct ChunkWords {
+    uint32_t w[8 * EB];
+};
+template <int EB>
+__device__ __noinline__ uint32_t chunk_statistics_general(ChunkWords<EB> cw, int jq, int jlim, uint8_t* dump_row,
+                                                          uint32_t sinks) {
     uint32_t zeros = 0;
 #pragma unroll
     for (int e = 0; e < 32; ++e) {
         uint32_t code;
         if constexpr (EB == 1) {
-            code = (w[e >> 2] >> (8 * (e & 3))) & 0xFFu;
+            code = (cw.w[e >> 2] >> (8 * (e & 3))) & 0xFFu;
         } else {
             uint32_t back;
-            asm("mul.rn.bf16x2 %0, %1, %2;" : "=r"(back) : "r"(w[e >> 1]), "r"(0x03800380u));   // 2^-120
+            asm("mul.rn.bf16x2 %0, %1, %2;" : "=r"(back) : "r"(cw.w[e >> 1]), "r"(0x03800380u));   // 2^-120
             code = (back >> (16 * (e & 1) + 4)) & 0xFFu;
         }
         const bool vis = jq + e <= jlim;
         if (vis && dump_row != nullptr) dump_row[jq + e] = (uint8_t)code;
         if (vis && code == 0 && !((sinks >> e) & 1u)) ++zeros;
     }
-    if (uf != nullptr) *uf += zeros;
+    return zeros;
+}
+template <int EB>
+__device__ __forceinline__ uint32_t chunk_statistics(const uint32_t* w, int jq, int jlim, uint8_t* dump_row, bool count,
+                                                     const FwdParams& p, bool sink_blk) {
+    constexpr int NW = 8 * EB;      // words of the chunk
+    if (dump_row == nullptr && !count) return 0u;
+    // which keys of the chunk are sink keys (sink_blk: the KV block of the chunk holds one at all)
+    const uint32_t sinks = sink_blk ? sink_mask32(p, jq) : 0u;
+    if (dump_row == nullptr && sinks == 0u && jq + 31 <= jlim) {
+        // every key of the chunk is visible and none is a sink: count the NON-zero codes a word at a time.  P >= 0,
+        // so a code is at most 0x7E (a BF16 value at most 0x7FFF) and adding 0x7F.. sets the top bit of exactly the
+        // non-zero lanes without a carry between them; no popc (it shares the MUFU pipe with ex2)
+        uint32_t nz = 0;
+#pragma unroll
+        for (int i = 0; i < NW; ++i) {
+            if constexpr (EB == 1) nz = __dp4a((w[i] + 0x7F7F7F7Fu) & 0x80808080u, 0x01010101u, nz);   // += 128 per code
+            else nz += ((w[i] + 0x7FFF7FFFu) >> 15) & 0x00010001u;
+        }
+        return 32u - ((EB == 1) ? (nz >> 7) : ((nz & 0xFFFFu) + (nz >> 16)));
+    }
+    ChunkWords<EB> cw;
+#pragma unroll
+    for (int i = 0; i < NW; ++i) cw.w[i] = w[i];
+    const uint32_t zeros = chunk_statistics_general<EB>(cw, jq, jlim, dump_row, sinks);
+    return count ? zeros : 0u;
 }
 
 }  // namespace fp8attn
