@@ -51,7 +51,12 @@ int check_device() {
     static std::mutex mu;
     static int cached_dev = -1, cached_rc = 0;
     std::lock_guard<std::mutex> lock(mu);
-    if (dev == cached_dev) return cached_rc;
+    static int cached_major = 0;
+    if (dev == cached_dev) {
+        // (the message is per thread: write it again for a caller that did not make the first query)
+        if (cached_rc) set_err("device %d has compute capability %d.x; sm_100 is required", dev, cached_major);
+        return cached_rc;
+    }
     int major = 0;
     if (cudaDeviceGetAttribute(&major, cudaDevAttrComputeCapabilityMajor, dev) != cudaSuccess) {
         cudaGetLastError();
@@ -59,6 +64,7 @@ int check_device() {
         return FP8ATTN_E_DEVICE;
     }
     cached_dev = dev;
+    cached_major = major;
     cached_rc = (major == 10) ? FP8ATTN_OK : FP8ATTN_E_DEVICE;
     if (cached_rc) set_err("device %d has compute capability %d.x; sm_100 is required", dev, major);
     return cached_rc;
