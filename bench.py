@@ -365,7 +365,8 @@ def run_ours(args, rank, world, dev):
     line = {
         "metric": "FP8 attention forward throughput" if bound == "tensor" else "split-KV decode attention bandwidth",
         "value": value, "unit": unit, "n_gpus": world, "steps": args.steps, "warmup": max(args.warmup, 3),
-        "ms_per_step": ms, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+        "ms_per_step": ms, "ms_median": float(np.median(per_step)), "ms_best": float(np.min(per_step)),
+        "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
         "dtype": "e4m3 (fp32 accumulate)" if mode == 2 else "bf16 (fp32 accumulate), P cast to e4m3",
         "data": "synthetic",
         "config": config_of(args.workload, r.block_m, r.block_n, r.num_splits),
@@ -556,7 +557,8 @@ def run_ours_extra(args, dev):
 
     per_step, total_ms, clocks, r = timed_steps(step, args.steps, 3, dev)
     ms = total_ms / args.steps
-    out = {"value": amount / (ms * 1e-3), "unit": unit, "ms_per_step": ms, "steps": args.steps, "kernel_id": r.kernel_id,
+    out = {"value": amount / (ms * 1e-3), "unit": unit, "ms_per_step": ms, "ms_median": float(np.median(per_step)),
+           "ms_best": float(np.min(per_step)), "steps": args.steps, "kernel_id": r.kernel_id,
            "num_splits": r.num_splits, "block_n": r.block_n, "gpu_launches_per_step": r.n_launches,
            "dtype": "e4m3 (fp32 accumulate)" if mode == 2 else "bf16 (fp32 accumulate), P cast to e4m3",
            "config": config_of(args.workload, r.block_m, r.block_n, r.num_splits),
