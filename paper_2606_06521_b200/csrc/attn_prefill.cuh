@@ -250,6 +250,25 @@ __device__ __forceinline__ void p_quarter(const uint32_t* v, uint32_t tS, int qu
     if constexpr (AUX) zeros += chunk_statistics<EB>(w, j0 + quarter * 32, jlim, dump_row, count, p, sink_blk);
 }
 
+// Lines 8-9 of one P quarter whose exp_part is done: sum / cast (cast_part), P over the head of its S quarter in TMEM,
+// arrival on the issuer's barrier, then the statistics (AUX).
+template <int EB, bool FOLD, bool AUX>
+__device__ __forceinline__ void p_quarter_finish(const float* pr, uint32_t tS, int quarter, int j0, int jlim, uint64_t s_2,
+                                                 uint64_t& sum_a, uint64_t& sum_b, uint64_t* bar, int lane,
+                                                 uint8_t* dump_row, bool count, uint32_t& zeros, const FwdParams& p,
+                                                 bool sink_blk) {
+    using C = PrefillCfg<EB>;
+    uint32_t w[C::P_COLS / 4];
+    cast_part<EB, FOLD>(pr, w, s_2, sum_a, sum_b);
+    if constexpr (EB == 1) ptx::tmem_st_x8(tS + quarter * 32, w);
+    else ptx::tmem_st_x16(tS + quarter * 32, w);
+    ptx::tmem_wait_st();
+    ptx::tc_fence_before();
+    __syncwarp();
+    if (lane == 0) ptx::mbar_arrive(bar);
+    if constexpr (AUX) zeros += chunk_statistics<EB>(w, j0 + quarter * 32, jlim, dump_row, count, p, sink_blk);
+}
+
 // ---- exp warp (wq, half): Alg. 1 lines 7-9 and 12 for its rows of both tiles, its 64 key columns ----
 template <int EB, bool FOLD, bool AUX, bool EXT>
 __device__ __forceinline__ void prefill_exp_warp(const FwdParams& p, int wq, int half, int lane, uint32_t tbase,
@@ -333,15 +352,19 @@ __device__ __forceinline__ void prefill_exp_warp(const FwdParams& p, int wq, int
             // exist and are not counted
             const bool sink_blk = AUX && sink_in_range(p, j0, 128);
             uint32_t zeros = 0;
-            p_quarter<EB, FOLD, CK::NPOLY, AUX>(r, tS, 2 * half, j0, jlim[t], cl2_2, negm_2, s_2, sum_a, sum_b,
-                                                p_full + 2 * t + 0, lane, dump_row[t], count_row[t], zeros, p, sink_blk);
+            // line 7 of both quarters first (in place: the logits become P), then lines 8-9 and the hand-off of each:
+            // the MUFU pipe works on the second quarter while the first one is cast, stored and handed over
+            float* const pr = reinterpret_cast<float*>(r);
+            exp_part<false, CK::NPOLY>(r, pr, j0 + half * 64, jlim[t], cl2_2, negm_2);
+            exp_part<false, CK::NPOLY>(r + 32, pr + 32, j0 + half * 64 + 32, jlim[t], cl2_2, negm_2);
+            p_quarter_finish<EB, FOLD, AUX>(pr, tS, 2 * half, j0, jlim[t], s_2, sum_a, sum_b, p_full + 2 * t + 0, lane,
+                                            dump_row[t], count_row[t], zeros, p, sink_blk);
             if (probe_next) {
                 ptx::mbar_probe(m_full + 4 * (t ^ 1) + wq, c_o & 1);
                 probed_tile = t ^ 1;
             }
-            p_quarter<EB, FOLD, CK::NPOLY, AUX>(r + 32, tS, 2 * half + 1, j0, jlim[t], cl2_2, negm_2, s_2, sum_a,
-                                                sum_b, p_full + 2 * t + 1, lane, dump_row[t], count_row[t], zeros, p,
-                                                sink_blk);
+            p_quarter_finish<EB, FOLD, AUX>(pr + 32, tS, 2 * half + 1, j0, jlim[t], s_2, sum_a, sum_b, p_full + 2 * t + 1,
+                                            lane, dump_row[t], count_row[t], zeros, p, sink_blk);
             if constexpr (AUX) {
                 if (sink_blk) uf_sink += zeros;
                 else uf_other += zeros;

@@ -61,10 +61,13 @@ __device__ __forceinline__ void exp2_poly2(uint64_t x2, float& r0, float& r1) {
 // pre-cast P (times S when the scale is folded into the exponent) to the two packed sums.
 // NPOLY: bit i set = element pair i of the 16 pairs of the chunk takes exp2_poly2 instead of ex2.approx
 // (0: all on the MUFU pipe).
-template <int EB, bool FOLD, bool MASK, int NPOLY = 0>
-__device__ __forceinline__ void exp_chunk(const uint32_t* v, uint32_t* w, int j_first, int jlim, uint64_t cl2_2,
-                                          uint64_t negm_2, uint64_t s_2, uint64_t& sum_a, uint64_t& sum_b) {
-    float pr[32];
+// The two halves of exp_chunk: exp_part is line 7 (P = exp2 of the scaled, shifted logit; FP32), cast_part lines 8-9
+// (row sum from the pre-cast P, the cast, the packing).  The exp warps of attn_prefill.cuh run the exp_part of BOTH
+// their quarters first and the cast_part + hand-off of each afterwards, so that the MUFU pipe works on the second
+// quarter while the first one is cast, stored and handed over.
+template <bool MASK, int NPOLY>
+__device__ __forceinline__ void exp_part(const uint32_t* v, float* pr, int j_first, int jlim, uint64_t cl2_2,
+                                         uint64_t negm_2) {
 #pragma unroll
     for (int e = 0; e < 32; e += 2) {
         uint32_t a = v[e], b = v[e + 1];
@@ -82,6 +85,9 @@ __device__ __forceinline__ void exp_chunk(const uint32_t* v, uint32_t* w, int j_
             pr[e + 1] = ptx::ex2_approx(x1);
         }
     }
+}
+template <int EB, bool FOLD>
+__device__ __forceinline__ void cast_part(const float* pr, uint32_t* w, uint64_t s_2, uint64_t& sum_a, uint64_t& sum_b) {
     uint32_t pair[16];
 #pragma unroll
     for (int e = 0; e < 32; e += 4) {
@@ -107,6 +113,13 @@ __device__ __forceinline__ void exp_chunk(const uint32_t* v, uint32_t* w, int j_
 #pragma unroll
         for (int e = 0; e < 16; ++e) w[e] = e4m3x2_to_bf16x2(pair[e]);
     }
+}
+template <int EB, bool FOLD, bool MASK, int NPOLY = 0>
+__device__ __forceinline__ void exp_chunk(const uint32_t* v, uint32_t* w, int j_first, int jlim, uint64_t cl2_2,
+                                          uint64_t negm_2, uint64_t s_2, uint64_t& sum_a, uint64_t& sum_b) {
+    float pr[32];
+    exp_part<MASK, NPOLY>(v, pr, j_first, jlim, cl2_2, negm_2);
+    cast_part<EB, FOLD>(pr, w, s_2, sum_a, sum_b);
 }
 
 // max over 32 (masked) raw logits folded into m
