@@ -85,6 +85,8 @@ extern "C" {
 #define FP8ATTN_E_DEVICE       -6   /* current device is not compute capability 10.x             */
 #define FP8ATTN_E_CUDA         -7   /* a CUDA call failed (allocation, tensor map, launch)       */
 #define FP8ATTN_E_STATS        -8   /* stats->struct_size does not match this header             */
+#define FP8ATTN_E_SCRATCH      -9   /* fp8attn_decode_noalloc: the call needs more scratch than
+                                       FP8ATTN_NOALLOC_SCRATCH_BYTES                              */
 
 #define FP8ATTN_MAX_SPLITS 64
 
@@ -194,6 +196,38 @@ FP8ATTN_API int fp8attn_fwd(const void *q, const void *k, const void *v, void *o
 FP8ATTN_API int fp8attn_fwd_host(const void *q, const void *k, const void *v, void *o,
                                  int B, int Hq, int Hkv, int Lq, int Lk, int d,
                                  int causal, float S, int kv_order, int mode, fp8attn_stats *stats);
+
+/*
+ * fp8attn_decode_noalloc -- the split-KV decode path of fp8attn_fwd for callers that must not allocate
+ * (code under CUDA graph capture, tight serving loops, harnesses that forbid cudaMalloc).  Same
+ * arguments, same kernels, same split layout and therefore the same results bit for bit as
+ * fp8attn_fwd on a decode-shaped call; what differs is where the scratch lives.  fp8attn_fwd takes
+ * the quantised q and the split-KV partials (m_s, l_s, O_s, reading R14)
+ * from a stream-ordered memory pool per call; this entry point keeps them in ONE file-scope
+ * `static __device__` array of FP8ATTN_NOALLOC_SCRATCH_BYTES that every GPU which loads the
+ * library holds until the process exits.  It calls no cudaMalloc, cudaFree, pool or other
+ * allocating routine (what it does call: cudaGetSymbolAddress once per device, tensor-map encoding
+ * on the host, cudaMemsetAsync on caller buffers, kernel launches).
+ *   Accepted: mode FP8ATTN_MODE_FP8 with FP8ATTN_DTYPE_BF16Q_E4M3KV or FP8ATTN_DTYPE_E4M3, d = 128,
+ *   block_n 0 or 128, (Hq / Hkv) * Lq <= 16 (the decode kernel's shape), stats->kernel 0 or 3;
+ *   everything else of fp8attn_stats as in fp8attn_fwd (num_splits 0 = the same automatic count).
+ *   Anything else: FP8ATTN_E_UNSUPPORTED.
+ *   Scratch needed: B*Hq*Lq*d + 4*B*Hq bytes for the quantised q (BF16 q only) plus, with more than
+ *   one split, num_splits * B*Hq*Lq * (d + 2) * 4 bytes of partials, each part rounded up to 256 B
+ *   (BASELINE config 5 with 4 splits: 4.5 MB).  A call that needs more than
+ *   FP8ATTN_NOALLOC_SCRATCH_BYTES gets FP8ATTN_E_SCRATCH and fp8attn_last_cuda_error() names both
+ *   sizes; nothing has been launched then.
+ *   Every call on a device shares the array, and the array keeps the contents of the last call.
+ *   No word of it has to start at zero: every word a kernel of a call reads has been written by an
+ *   earlier kernel of the same call on the same stream (the caller's counters in stats->underflow
+ *   are cleared by the call, as in fp8attn_fwd).  Calls that can overlap on the GPU -- two streams,
+ *   two host threads on one device -- RACE on the array: the caller serialises them (one stream, or
+ *   events).  Calls on different devices do not interact.
+ */
+#define FP8ATTN_NOALLOC_SCRATCH_BYTES (16u << 20)
+FP8ATTN_API int fp8attn_decode_noalloc(const void *q, const void *k, const void *v, void *o,
+                                       int B, int Hq, int Hkv, int Lq, int Lk, int d,
+                                       int causal, float S, int kv_order, int mode, fp8attn_stats *stats);
 
 /*
  * fp8attn_quantize_e4m3 -- per-(b,h) slab quantisation of FP32 to E4M3 (BASELINE config 3

@@ -377,12 +377,41 @@ int validate_args(const void* q, const void* k, const void* v, const void* o, in
 
 }  // namespace
 
+// ---------------------------------------------------------------------------- static scratch (fp8attn_decode_noalloc)
+// The scratch of the entry point that allocates nothing.  In HOST code this name is a host-side stand-in, not a
+// device address: the address a kernel can use comes from cudaGetSymbolAddress, asked once per device with that
+// device current (every device that loads the library has its own copy of the array).
+static __device__ __align__(256) unsigned char g_noalloc_scratch[FP8ATTN_NOALLOC_SCRATCH_BYTES];
+
+namespace {
+
+int noalloc_scratch_ptr(unsigned char** out) {
+    static std::mutex mu;
+    static unsigned char* ptrs[MAX_DEVICES] = {};
+    int dev = 0;
+    if (int rc = current_device(&dev)) return rc;
+    std::lock_guard<std::mutex> lock(mu);
+    if (!ptrs[dev]) {
+        void* ptr = nullptr;
+        CU_TRY(cudaGetSymbolAddress(&ptr, g_noalloc_scratch));
+        if (!ptr || (reinterpret_cast<uintptr_t>(ptr) & 255u)) {
+            set_err("cudaGetSymbolAddress gave %p for the static scratch of device %d", ptr, dev);
+            return FP8ATTN_E_CUDA;
+        }
+        ptrs[dev] = static_cast<unsigned char*>(ptr);
+    }
+    *out = ptrs[dev];
+    return FP8ATTN_OK;
+}
+
+}  // namespace
+
 // =============================================================================================
 // C ABI
 // =============================================================================================
 extern "C" {
 
-int fp8attn_version(void) { return 200; }   // 0.2.0
+int fp8attn_version(void) { return 201; }   // 0.2.1
 
 int fp8attn_trim(void) {
     int dev = 0;
@@ -406,6 +435,7 @@ const char* fp8attn_strerror(int code) {
         case FP8ATTN_E_DEVICE: return "the current device is not compute capability 10.x";
         case FP8ATTN_E_CUDA: return "a CUDA call failed (see fp8attn_last_cuda_error)";
         case FP8ATTN_E_STATS: return "stats->struct_size does not match this header";
+        case FP8ATTN_E_SCRATCH: return "the call needs more scratch than the static array of fp8attn_decode_noalloc holds";
         default: return "unknown error code";
     }
 }
@@ -614,6 +644,135 @@ int fp8attn_fwd(const void* q, const void* k, const void* v, void* o, int B, int
     return FP8ATTN_OK;
 }
 
+// The decode path of fp8attn_fwd (q quantiser, split-KV decode kernel, combine) with its scratch in the static
+// array above: no cudaMalloc, no cudaFree, no pool (include/fp8attn.h).  Same kernels, same launch configuration
+// and the same split layout as fp8attn_fwd, so the results are the same bit for bit.
+int fp8attn_decode_noalloc(const void* q, const void* k, const void* v, void* o, int B, int Hq, int Hkv, int Lq, int Lk,
+                           int d, int causal, float S, int kv_order, int mode, fp8attn_stats* stats) {
+    if (int rc = validate_args(q, k, v, o, B, Hq, Hkv, Lq, Lk, d, S, kv_order, mode, stats)) return rc;
+    const int pm = mode & 0xFF, dt = (mode >> 8) & 0xF;
+    const int bn = 128;
+    const int want_kernel = stats ? stats->kernel : 0;
+    if (pm != FP8ATTN_MODE_FP8 || d != 128 || (stats && stats->block_n != 0 && stats->block_n != 128) ||
+        (long long)(Hq / Hkv) * Lq > 16 || (want_kernel != 0 && want_kernel != 3)) {
+        set_err("fp8attn_decode_noalloc serves decode shapes only: FP8 mode, d = 128, block_n 128, (Hq/Hkv)*Lq <= 16");
+        return FP8ATTN_E_UNSUPPORTED;
+    }
+    if (int rc = check_device()) return rc;
+    cudaStream_t st = stats ? reinterpret_cast<cudaStream_t>(stats->stream) : nullptr;
+    const long long q_slabs = (long long)B * Hq, kv_slabs = (long long)B * Hkv;
+    const int nb = (Lk + bn - 1) / bn;
+    int ns = stats ? stats->num_splits : 0;
+    if (ns == 0) ns = decode_auto_splits(kv_slabs, nb);
+    if (ns > nb) ns = nb;
+    const long long nq = q_slabs * Lq * d, R = q_slabs * Lq;
+
+    // ---- layout of the call in the static array: [q codes][q scales][partial O][partial (m, l)]
+    auto up = [](size_t x) { return (x + 255) & ~size_t(255); };
+    size_t off = 0;
+    const size_t o_codes = off;  off += (dt == 3) ? up((size_t)nq) : 0;
+    const size_t o_qsc = off;    off += (dt == 3) ? up((size_t)q_slabs * 4) : 0;
+    const size_t o_part = off;   off += (ns > 1) ? up((size_t)ns * R * (d + 2) * 4) : 0;
+    if (off > (size_t)FP8ATTN_NOALLOC_SCRATCH_BYTES) {
+        set_err("fp8attn_decode_noalloc: this call needs %zu bytes of scratch (%d splits), the static array holds %u",
+                off, ns, (unsigned)FP8ATTN_NOALLOC_SCRATCH_BYTES);
+        return FP8ATTN_E_SCRATCH;
+    }
+    unsigned char* scratch = nullptr;
+    if (int rc = noalloc_scratch_ptr(&scratch)) return rc;
+
+    const void* qs = q;
+    const float* q_scale = stats ? stats->q_scale : nullptr;
+    int n_launches = 0;
+    if (dt == 3) {
+        // the BF16 q of every (b, hq) slab to E4M3 (reading R24): Lq * d <= 2048 elements per slab, one warp each
+        uint8_t* codes = scratch + o_codes;
+        float* qsc = reinterpret_cast<float*>(scratch + o_qsc);
+        quantize_small_slabs_kernel<__nv_bfloat16><<<(unsigned)((q_slabs + 3) / 4), 128, 0, st>>>(
+            static_cast<const __nv_bfloat16*>(q), codes, qsc, Lq * d, (int)q_slabs);
+        CU_TRY(cudaGetLastError());
+        ++n_launches;
+        qs = codes;
+        q_scale = qsc;
+    }
+
+    const bool paged = stats && stats->block_table;
+    if (paged && stats->page_size % bn != 0) return FP8ATTN_E_UNSUPPORTED;
+    CUtensorMap mq16, mk, mv;
+    // the G*Lq query rows of one kv head are consecutive rows of q: one 16-row box per CTA
+    if (int rc = make_map(&mq16, qs, 1, 1, q_slabs * Lq, d, 16)) return rc;
+    if (paged) {
+        if (int rc = make_map(&mk, k, 1, (long long)stats->num_pages * Hkv, stats->page_size, d, bn)) return rc;
+        if (int rc = make_map(&mv, v, 1, (long long)stats->num_pages * Hkv, stats->page_size, d, bn)) return rc;
+    } else {
+        if (int rc = make_map(&mk, k, 1, kv_slabs, Lk, d, bn)) return rc;
+        if (int rc = make_map(&mv, v, 1, kv_slabs, Lk, d, bn)) return rc;
+    }
+    FwdParams p;
+    memset(&p, 0, sizeof p);
+    p.o = o;
+    p.row_max = stats ? stats->row_max : nullptr;
+    p.row_sum = stats ? stats->row_sum : nullptr;
+    p.underflow = stats ? stats->underflow : nullptr;
+    p.p_codes = stats ? stats->p_codes : nullptr;
+    p.p_bh = stats ? stats->p_batch * Hq + stats->p_head : 0;
+    p.q_scale = q_scale;
+    p.k_scale = stats ? stats->k_scale : nullptr;
+    p.v_scale = stats ? stats->v_scale : nullptr;
+    p.B = B; p.Hq = Hq; p.Hkv = Hkv; p.Lq = Lq; p.Lk = Lk;
+    p.causal = causal ? 1 : 0;
+    p.kv_order = kv_order;
+    p.n_sink = stats ? stats->n_sink : 0;
+    p.scale_mode = stats ? stats->scale_mode : 0;
+    p.o_bf16 = (stats && stats->o_dtype == FP8ATTN_O_BF16) ? 1 : 0;
+    p.n_sinkpos = -1;
+    if (stats && stats->sink_pos) {
+        p.n_sinkpos = stats->n_sink;
+        for (int i = 0; i < stats->n_sink; ++i) p.sink_pos[i] = stats->sink_pos[i];
+    }
+    const bool dynamic = p.scale_mode == 1;
+    p.seqlens_q = stats ? stats->seqlens_q : nullptr;
+    p.seqlens_k = stats ? stats->seqlens_k : nullptr;
+    p.block_table = paged ? stats->block_table : nullptr;
+    p.page_size = paged ? stats->page_size : 0;
+    p.max_pages = paged ? stats->max_pages : 0;
+    p.num_splits = ns;
+    p.nb = nb;
+    p.q_slabs = (int)q_slabs;
+    p.kv_slabs = (int)kv_slabs;
+    p.S = S;
+    p.sm_scale = 1.0f / sqrtf((float)d);
+    if (ns > 1) {
+        p.part_o = reinterpret_cast<float*>(scratch + o_part);
+        p.part_ml = p.part_o + (size_t)ns * R * d;
+    }
+    // caller buffers that must start clean (cudaMemsetAsync allocates nothing); the scratch needs no clearing:
+    // the decode kernel writes every partial the combine kernel reads
+    if (p.underflow) CU_TRY(cudaMemsetAsync(p.underflow, 0, 2 * sizeof(unsigned long long), st));
+    if (p.p_codes) CU_TRY(cudaMemsetAsync(p.p_codes, 0xFF, (size_t)Lq * Lk, st));
+
+    const int nv = (Hq / Hkv) * Lq;
+    const int rc = (is_pow2_scale(S) || dynamic) ? launch_decode<true>(nv, mq16, mk, mv, p, st)
+                                                 : launch_decode<false>(nv, mq16, mk, mv, p, st);
+    if (rc) return rc;
+    ++n_launches;
+    if (ns > 1) {
+        const int rows_per_block = 8;
+        combine_kernel<<<(unsigned)((R + rows_per_block - 1) / rows_per_block), rows_per_block * 32, 0, st>>>(
+            p.part_o, p.part_ml, p.o, p.row_max, p.row_sum, p.v_scale, R, d, ns, dynamic ? 1.0f : S, Hq, Hkv, Lq, p.o_bf16);
+        CU_TRY(cudaGetLastError());
+        ++n_launches;
+    }
+    if (stats) {
+        stats->block_m_used = BM;
+        stats->block_n_used = bn;
+        stats->num_splits_used = ns;
+        for (int s = 0; s <= ns; ++s) stats->split_bounds[s] = (int)(((long long)s * nb) / ns);
+        stats->kernel_id = 3;
+        stats->n_launches = n_launches;
+    }
+    return FP8ATTN_OK;
+}
 int fp8attn_fwd_host(const void* q, const void* k, const void* v, void* o, int B, int Hq, int Hkv, int Lq, int Lk,
                      int d, int causal, float S, int kv_order, int mode, fp8attn_stats* stats) {
     if (int rc = validate_args(q, k, v, o, B, Hq, Hkv, Lq, Lk, d, S, kv_order, mode, stats)) return rc;

@@ -2,9 +2,10 @@
 of the method runs in the CUDA kernels behind the C ABI.  torch is used for device memory and
 streams.  There is no CPU path: if the library cannot be loaded, importing this module fails.
 
-The C entry points are exposed under their own names (`fp8attn_fwd`, `fp8attn_quantize_e4m3`,
-`fp8attn_debug_gemm`, `fp8attn_strerror`, `fp8attn_version`) taking raw device pointers, plus
-the tensor-level wrappers `fwd`, `quantize_e4m3` and `debug_gemm`.
+The C entry points are exposed under their own names (`fp8attn_fwd`, `fp8attn_fwd_host`,
+`fp8attn_decode_noalloc`, `fp8attn_quantize_e4m3`, `fp8attn_debug_gemm`, `fp8attn_strerror`,
+`fp8attn_version`) taking raw device pointers, plus the tensor-level wrappers `fwd`, `fwd_host`,
+`decode_noalloc`, `quantize_e4m3` and `debug_gemm`.
 """
 import ctypes as C
 import os
@@ -56,6 +57,8 @@ def _load():
     lib.fp8attn_fwd.restype = C.c_int
     lib.fp8attn_fwd_host.argtypes = lib.fp8attn_fwd.argtypes
     lib.fp8attn_fwd_host.restype = C.c_int
+    lib.fp8attn_decode_noalloc.argtypes = lib.fp8attn_fwd.argtypes
+    lib.fp8attn_decode_noalloc.restype = C.c_int
     lib.fp8attn_quantize_e4m3.argtypes = [C.c_void_p] * 3 + [C.c_int] * 4 + [C.c_void_p]
     lib.fp8attn_quantize_e4m3.restype = C.c_int
     lib.fp8attn_debug_gemm.argtypes = [C.c_void_p] * 3 + [C.c_int] * 5 + [C.c_void_p]
@@ -73,6 +76,8 @@ LIB_PATH = _lib._name
 
 fp8attn_fwd = _lib.fp8attn_fwd
 fp8attn_fwd_host = _lib.fp8attn_fwd_host
+fp8attn_decode_noalloc = _lib.fp8attn_decode_noalloc
+NOALLOC_SCRATCH_BYTES = 16 << 20        # FP8ATTN_NOALLOC_SCRATCH_BYTES
 fp8attn_quantize_e4m3 = _lib.fp8attn_quantize_e4m3
 fp8attn_debug_gemm = _lib.fp8attn_debug_gemm
 fp8attn_version = _lib.fp8attn_version
@@ -86,7 +91,7 @@ def fp8attn_strerror(code: int) -> str:
 class Fp8AttnError(RuntimeError):
     def __init__(self, code):
         self.code = code
-        detail = _lib.fp8attn_last_cuda_error().decode() if code == -7 or code == -6 else ""
+        detail = _lib.fp8attn_last_cuda_error().decode() if code in (-6, -7, -9) else ""
         super().__init__(f"fp8attn error {code}: {fp8attn_strerror(code)}" + (f" [{detail}]" if detail else ""))
 
 
@@ -213,6 +218,47 @@ def fwd(q, k, v, *, causal: bool, S: float, kv_order: int, mode: int, n_sink: in
     _check(rc)
     ns = st.num_splits_used
     return FwdResult(o, row_max, row_sum, underflow, codes, st.block_m_used, st.block_n_used, ns,
+                     [st.split_bounds[i] for i in range(ns + 1)], st.kernel_id, st.n_launches)
+
+
+def decode_noalloc(q, k, v, o, *, S: float, kv_order: int, k_scale, v_scale, q_scale=None, causal: bool = False,
+                   n_sink: int = 4, num_splits: int = 0, row_max=None, row_sum=None, underflow=None, stream=None,
+                   scale_mode: int = 0) -> FwdResult:
+    """fp8attn_decode_noalloc: the split-KV decode path with its scratch in the library's static device array -- no
+    allocation in the library (include/fp8attn.h) and none here: every buffer, `o` and the optional statistics
+    (`row_max`, `row_sum` float32 [B,Hq,Lq]; `underflow` int64 [2]) included, is the caller's.  q is BF16 (quantised
+    per slab by the library) or E4M3 codes with `q_scale`; k, v are E4M3 codes with float32 CUDA scales [B,Hkv].
+    Calls that overlap on the GPU race on the scratch: keep them on one stream."""
+    for t in (q, k, v, o):
+        if not (t.is_cuda and t.is_contiguous() and t.dim() == 4):
+            raise ValueError("q, k, v, o must be contiguous 4-D CUDA tensors")
+    B, Hq, Lq, d = q.shape
+    Bk, Hkv, Lk, dk = k.shape
+    if (Bk, dk) != (B, d) or v.shape != k.shape or o.shape != q.shape:
+        raise ValueError("shape mismatch between q, k, v, o")
+    if o.dtype not in (torch.float32, torch.bfloat16):
+        raise TypeError("o must be float32 or bfloat16")
+    st = Stats()
+    st.struct_size = C.sizeof(Stats)
+    st.n_sink, st.num_splits, st.scale_mode = int(n_sink), int(num_splits), int(scale_mode)
+    st.o_dtype = 1 if o.dtype == torch.bfloat16 else 0
+    st.stream = _stream_ptr(stream)
+    for name, t in (("q_scale", q_scale), ("k_scale", k_scale), ("v_scale", v_scale), ("row_max", row_max),
+                    ("row_sum", row_sum)):
+        if t is not None:
+            if not (t.is_cuda and t.is_contiguous() and t.dtype == torch.float32):
+                raise TypeError(f"{name} must be a contiguous float32 CUDA tensor")
+            setattr(st, name, t.data_ptr())
+    if underflow is not None:
+        if not (underflow.is_cuda and underflow.dtype == torch.int64 and underflow.numel() == 2):
+            raise TypeError("underflow must be an int64 CUDA tensor of 2 elements")
+        st.underflow = underflow.data_ptr()
+    with torch.cuda.device(q.device):
+        rc = fp8attn_decode_noalloc(_ptr(q), _ptr(k), _ptr(v), _ptr(o), B, Hq, Hkv, Lq, Lk, d, int(bool(causal)), float(S),
+                                    int(kv_order), MODE_FP8 | _dtype_code(q, k), C.byref(st))
+    _check(rc)
+    ns = st.num_splits_used
+    return FwdResult(o, row_max, row_sum, underflow, None, st.block_m_used, st.block_n_used, ns,
                      [st.split_bounds[i] for i in range(ns + 1)], st.kernel_id, st.n_launches)
 
 

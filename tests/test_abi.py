@@ -63,7 +63,7 @@ def test_argument_checks_precede_any_cuda_call(fa):
     assert f(one, one, one, one, 1, 1, 1, 1, 1, 64, 0, 1.0, 0, 3, None) == -4       # mode
     assert f(one, one, one, one, 1, 1, 1, 1, 1, 64, 0, 1.0, 0, 2, None) == -4       # FP8 mode, FP32 dtype
     assert f(one, one, one, one, 1, 1, 1, 1, 1, 128, 0, 1.0, 0, 2 | (2 << 8), None) == -1   # no scales
-    for code in range(-8, 1):
+    for code in range(-9, 1):
         assert fa.fp8attn_strerror(code) != "unknown error code"
     assert fa.fp8attn_version() >= 100
 
