@@ -91,15 +91,20 @@ __device__ __forceinline__ bool mbar_test_wait(uint64_t* bar, uint32_t parity) {
         : "memory");
     return ok != 0;
 }
-// Wait for the phase with the given parity to complete.  Traps (instead of hanging) if the
-// barrier never flips.
+// Wait for the phase with the given parity to complete.  Traps (instead of hanging) if the barrier never flips.
+// The trap path makes no call: a printf here (an ABI call) makes ptxas keep loop-invariant values of the caller on
+// the stack and reload them at the join after EVERY wait -- a local-memory round trip on the path barrier -> TMEM
+// load of each block (measured on cfg3, see profiles/r2_prefill_cfg3.md).  -DFP8ATTN_DEBUG_MBAR brings the
+// message back for debugging.
 __device__ __forceinline__ void mbar_wait(uint64_t* bar, uint32_t parity) {
     if (mbar_try_wait(bar, parity)) return;
     const long long t0 = clock64();
     while (!mbar_try_wait(bar, parity)) {
         if (clock64() - t0 > FP8ATTN_MBAR_TIMEOUT_CYCLES) {
+#ifdef FP8ATTN_DEBUG_MBAR
             printf("fp8attn: mbarrier timeout block (%d,%d,%d) thread %d bar %u parity %u\n", blockIdx.x,
                    blockIdx.y, blockIdx.z, threadIdx.x, smem_u32(bar), parity);
+#endif
             __trap();
         }
     }
