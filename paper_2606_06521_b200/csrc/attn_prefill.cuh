@@ -491,14 +491,16 @@ attn_prefill_kernel(const __grid_constant__ CUtensorMap mapQ, const __grid_const
     ptx::tc_fence_before();
     __syncthreads();
     ptx::tc_fence_after();
-    const uint32_t tbase = *tmem_slot;
-
+    // (every role reads the TMEM base address itself, after its setmaxnreg: a value defined up here is spilled by the
+    // register budget of the smallest role and would be reloaded from local memory at every use)
     if (warp < 8) {
         ptx::setmaxnreg_inc<C4::REG_EXP>();
+        const uint32_t tbase = ptx::ld_shared_u32(tmem_slot);
         prefill_exp_warp<EB, FOLD, AUX, EXT>(p, warp & 3, warp >> 2, lane, tbase, m_full, p_full, mstat, lsum, lscale, o_done, n_tile,
                                         n_it, pair, bh, kvh, &mapO, sK, sV);
     } else if (warp < 16) {
         ptx::setmaxnreg_dec<C4::REG_MAX>();
+        const uint32_t tbase = ptx::ld_shared_u32(tmem_slot);
         const int t = (warp - 8) >> 2, wq = warp & 3;
         prefill_max_warp<EB, FOLD, EXT>(p, t, wq, lane, tbase, s_full + t, m_full + 4 * t + wq, mstat + t * 2 * 128,
                                    lscale + t * 128, o_ready + t, n_tile[t], (pair * 2 + t) * BM, bh, kvh, lsum, o_done,
@@ -546,6 +548,7 @@ attn_prefill_kernel(const __grid_constant__ CUtensorMap mapQ, const __grid_const
             const uint32_t q_lo = ptx::smem_desc_lo(ptx::smem_u32(sQ + t * C::TILE), 16);
             const uint32_t k_lo = ptx::smem_desc_lo(ptx::smem_u32(sK), 16);
             const uint32_t v_lo = ptx::smem_desc_lo(ptx::smem_u32(sV), C::BN * 128);
+            const uint32_t tbase = ptx::ld_shared_u32(tmem_slot);
             const uint32_t tS = tbase + C::TM_S + t * 128, tO = tbase + C::TM_O + t * 128;
             const int first = (p.kv_order == 0) ? 0 : n_it - n_t;
             const int n_other = n_tile[t ^ 1];
@@ -619,7 +622,7 @@ attn_prefill_kernel(const __grid_constant__ CUtensorMap mapQ, const __grid_const
 
     ptx::tc_fence_before();
     __syncthreads();
-    if (warp == 16) ptx::tmem_dealloc(tbase, 512);
+    if (warp == 16) ptx::tmem_dealloc(ptx::ld_shared_u32(tmem_slot), 512);
 }
 
 }  // namespace fp8attn

@@ -44,6 +44,13 @@ __device__ __forceinline__ void st_shared_v2(const void* p, float a, float b) {
 __device__ __forceinline__ void st_shared_v4(const void* p, uint32_t a, uint32_t b, uint32_t c, uint32_t d) {
     asm volatile("st.shared.v4.b32 [%0], {%1, %2, %3, %4};" ::"r"(smem_u32(p)), "r"(a), "r"(b), "r"(c), "r"(d) : "memory");
 }
+// (volatile: the load stays where it is written -- a role reads its own copy of a value after its setmaxnreg instead
+// of inheriting one that the common prologue has spilled)
+__device__ __forceinline__ uint32_t ld_shared_u32(const void* p) {
+    uint32_t r;
+    asm volatile("ld.shared.u32 %0, [%1];" : "=r"(r) : "r"(smem_u32(p)) : "memory");
+    return r;
+}
 __device__ __forceinline__ float2 ld_shared_v2(const void* p) {
     float2 r;
     asm volatile("ld.shared.v2.f32 {%0, %1}, [%2];" : "=f"(r.x), "=f"(r.y) : "r"(smem_u32(p)) : "memory");
