@@ -58,9 +58,9 @@ struct RowStat {
 // (128-byte swizzle; FP32: two boxes of 32 floats, BF16: one box of 64) into the K / V ring -- no MMA reads it any
 // more once both tiles are done -- and stored with TMA (rows >= Lq are clipped by the map).  The four warps that can
 // read a 32-lane quarter of TMEM (two exp warps, the max warps of both tiles) take one (tile, half) each.
-template <int EB, bool FOLD>
+template <int EB, bool FOLD, typename OB>
 __device__ __forceinline__ void prefill_store_half(const FwdParams& p, int t, int half, int wq, int lane, uint32_t tbase,
-                                                   const float* lsum, const float* lscale, uint64_t* o_done, bool has_blocks,
+                                                   const float* lsum, const float* lscale, OB o_done, bool has_blocks,
                                                    bool other_has_blocks,
                                                    int row0, int bh, float vs, const CUtensorMap* mapO, uint8_t* stage,
                                                    bool write_row_sum) {
@@ -128,9 +128,10 @@ __device__ __forceinline__ void prefill_store_half(const FwdParams& p, int t, in
 // instance has none of that code (measured: 1.3 % of cfg3).
 template <int EB, bool FOLD, bool EXT>
 __device__ __forceinline__ void prefill_max_warp(const FwdParams& p, int t, int wq, int lane, uint32_t tbase,
-                                                 uint64_t* s_full_t, uint64_t* m_full_w, RowStat* mstat_t,
-                                                 float* lscale_t, uint64_t* o_ready_t, int n_t, int row0, int bh, int kvh,
-                                                 const float* lsum, uint64_t* o_done, int n_other, const CUtensorMap* mapO,
+                                                 ptx::SPtr<uint64_t> s_full_t, ptx::SPtr<uint64_t> m_full_w,
+                                                 ptx::SPtr<RowStat> mstat_t, float* lscale_t, ptx::SPtr<uint64_t> o_ready_t,
+                                                 int n_t, int row0, int bh, int kvh, const float* lsum,
+                                                 ptx::SPtr<uint64_t> o_done, int n_other, const CUtensorMap* mapO,
                                                  uint8_t* stage) {
     using C = PrefillCfg<EB>;
     const uint32_t tlane = tbase + (static_cast<uint32_t>(wq * 32) << 16);
@@ -232,9 +233,9 @@ __device__ __forceinline__ void prefill_max_warp(const FwdParams& p, int t, int 
 
 // One P quarter: exp / sum / cast (exp_chunk), statistics (AUX), P over the head of its S quarter in TMEM (the A
 // operand of P.V), arrival on the issuer's barrier.
-template <int EB, bool FOLD, int NPOLY, bool AUX>
+template <int EB, bool FOLD, int NPOLY, bool AUX, typename BAR>
 __device__ __forceinline__ void p_quarter(const uint32_t* v, uint32_t tS, int quarter, int j0, int jlim, uint64_t cl2_2,
-                                          uint64_t negm_2, uint64_t s_2, uint64_t& sum_a, uint64_t& sum_b, uint64_t* bar,
+                                          uint64_t negm_2, uint64_t s_2, uint64_t& sum_a, uint64_t& sum_b, BAR bar,
                                           int lane, uint8_t* dump_row, bool count, uint32_t& zeros, const FwdParams& p,
                                           bool sink_blk) {
     using C = PrefillCfg<EB>;
@@ -252,9 +253,9 @@ __device__ __forceinline__ void p_quarter(const uint32_t* v, uint32_t tS, int qu
 
 // Lines 8-9 of one P quarter whose exp_part is done: sum / cast (cast_part), P over the head of its S quarter in TMEM,
 // arrival on the issuer's barrier, then the statistics (AUX).
-template <int EB, bool FOLD, bool AUX>
+template <int EB, bool FOLD, bool AUX, typename BAR>
 __device__ __forceinline__ void p_quarter_finish(const float* pr, uint32_t tS, int quarter, int j0, int jlim, uint64_t s_2,
-                                                 uint64_t& sum_a, uint64_t& sum_b, uint64_t* bar, int lane,
+                                                 uint64_t& sum_a, uint64_t& sum_b, BAR bar, int lane,
                                                  uint8_t* dump_row, bool count, uint32_t& zeros, const FwdParams& p,
                                                  bool sink_blk) {
     using C = PrefillCfg<EB>;
@@ -272,9 +273,9 @@ __device__ __forceinline__ void p_quarter_finish(const float* pr, uint32_t tS, i
 // ---- exp warp (wq, half): Alg. 1 lines 7-9 and 12 for its rows of both tiles, its 64 key columns ----
 template <int EB, bool FOLD, bool AUX, bool EXT>
 __device__ __forceinline__ void prefill_exp_warp(const FwdParams& p, int wq, int half, int lane, uint32_t tbase,
-                                                 uint64_t* m_full, uint64_t* p_full, const RowStat* mstat, float* lsum,
-                                                 const float* lscale,
-                                                 uint64_t* o_done, const int* n_tile, int n_it, int pair, int bh,
+                                                 ptx::SPtr<uint64_t> m_full, ptx::SPtr<uint64_t> p_full,
+                                                 ptx::SPtr<RowStat> mstat, float* lsum, const float* lscale,
+                                                 ptx::SPtr<uint64_t> o_done, const int* n_tile, int n_it, int pair, int bh,
                                                  int kvh, const CUtensorMap* mapO, uint8_t* stage0, uint8_t* stage1) {
     using C = PrefillCfg<EB>;
     using CK = PrefillKCfg<EB>;
@@ -491,22 +492,40 @@ attn_prefill_kernel(const __grid_constant__ CUtensorMap mapQ, const __grid_const
     ptx::tc_fence_before();
     __syncthreads();
     ptx::tc_fence_after();
-    // (every role reads the TMEM base address itself, after its setmaxnreg: a value defined up here is spilled by the
-    // register budget of the smallest role and would be reloaded from local memory at every use)
+    // Every role reads the TMEM base address itself and builds its own 32-bit shared addresses from one opaque base
+    // register, after its setmaxnreg: a value defined up here is spilled by the register budget of the smallest
+    // role and reloaded from local memory at every use, and generic pointers into the aligned dynamic shared
+    // memory are rematerialised (S2UR window + align) at every barrier operation.
+    constexpr uint32_t OFF_BARS = (2 + 2 * C::NS) * C::TILE;
+    constexpr uint32_t OFF_MSTAT = OFF_BARS + C4::N_BARS * 8 + 16;
+    const auto shared_base = [&]() { return ptx::opaque_u32((ptx::smem_u32(smem_raw) + 1023u) & ~1023u); };
     if (warp < 8) {
         ptx::setmaxnreg_inc<C4::REG_EXP>();
         const uint32_t tbase = ptx::ld_shared_u32(tmem_slot);
-        prefill_exp_warp<EB, FOLD, AUX, EXT>(p, warp & 3, warp >> 2, lane, tbase, m_full, p_full, mstat, lsum, lscale, o_done, n_tile,
-                                        n_it, pair, bh, kvh, &mapO, sK, sV);
+        const ptx::SPtr<uint64_t> sbar{shared_base() + OFF_BARS};
+        const ptx::SPtr<RowStat> smstat{sbar.a + (OFF_MSTAT - OFF_BARS)};
+        prefill_exp_warp<EB, FOLD, AUX, EXT>(p, warp & 3, warp >> 2, lane, tbase, sbar + (8 + 4 * C::NS), sbar + (4 + 4 * C::NS),
+                                             smstat, lsum, lscale, sbar + (18 + 4 * C::NS), n_tile, n_it, pair, bh, kvh, &mapO,
+                                             sK, sV);
     } else if (warp < 16) {
         ptx::setmaxnreg_dec<C4::REG_MAX>();
         const uint32_t tbase = ptx::ld_shared_u32(tmem_slot);
+        const ptx::SPtr<uint64_t> sbar{shared_base() + OFF_BARS};
+        const ptx::SPtr<RowStat> smstat{sbar.a + (OFF_MSTAT - OFF_BARS)};
         const int t = (warp - 8) >> 2, wq = warp & 3;
-        prefill_max_warp<EB, FOLD, EXT>(p, t, wq, lane, tbase, s_full + t, m_full + 4 * t + wq, mstat + t * 2 * 128,
-                                   lscale + t * 128, o_ready + t, n_tile[t], (pair * 2 + t) * BM, bh, kvh, lsum, o_done,
-                                   n_tile[t ^ 1], &mapO, t ? sV : sK);
+        prefill_max_warp<EB, FOLD, EXT>(p, t, wq, lane, tbase, sbar + (2 + 4 * C::NS + t), sbar + (8 + 4 * C::NS + 4 * t + wq),
+                                        smstat + t * 2 * 128, lscale + t * 128, sbar + (16 + 4 * C::NS + t), n_tile[t],
+                                        (pair * 2 + t) * BM, bh, kvh, lsum, sbar + (18 + 4 * C::NS), n_tile[t ^ 1], &mapO,
+                                        t ? sV : sK);
     } else {
         ptx::setmaxnreg_dec<C4::REG_MISC>();
+        // the same barriers and tiles as 32-bit shared addresses (these names shadow the generic pointers above)
+        const uint32_t sb = shared_base();
+        const ptx::SPtr<uint8_t> sQ{sb}, sK{sb + 2 * C::TILE}, sV{sb + (2 + C::NS) * C::TILE};
+        const ptx::SPtr<uint64_t> q_full{sb + OFF_BARS};
+        const ptx::SPtr<uint64_t> k_full = q_full + 2, k_empty = k_full + C::NS, v_full = k_empty + C::NS,
+                                  v_empty = v_full + C::NS, s_full = v_empty + C::NS, p_full = s_full + 2,
+                                  o_ready = p_full + 12, o_done = o_ready + 2;
         if (warp == 18) {
             // ================= TMA producer =================
             if (lane == 0 && n_it > 0) {
@@ -553,7 +572,7 @@ attn_prefill_kernel(const __grid_constant__ CUtensorMap mapQ, const __grid_const
             const int first = (p.kv_order == 0) ? 0 : n_it - n_t;
             const int n_other = n_tile[t ^ 1];
             const int first_other = (p.kv_order == 0) ? 0 : n_it - n_other;
-            uint64_t* const pf = p_full + 2 * t;
+            const ptx::SPtr<uint64_t> pf = p_full + 2 * t;
 
             // S_t = Q_t K^T on ring iteration it
             // (the caller has waited for the K tile of ring iteration it: k_full)

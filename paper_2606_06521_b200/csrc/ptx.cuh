@@ -17,6 +17,26 @@ __device__ __forceinline__ uint32_t smem_u32(const void* p) {
     return static_cast<uint32_t>(__cvta_generic_to_shared(p));
 }
 
+// A 32-bit shared-memory address with pointer arithmetic.  The hot loops of the warp-specialised kernels address
+// their barriers and row statistics through these, built from ONE opaque base register per role: a generic pointer
+// derived from the aligned dynamic-shared-memory base is rematerialised by ptxas at every use (S2UR window + align,
+// a dozen dependent uniform instructions between a barrier wake and the TMEM load it guards).
+template <typename T>
+struct SPtr {
+    uint32_t a;
+    __device__ __forceinline__ SPtr operator+(int i) const { return SPtr{a + static_cast<uint32_t>(i) * static_cast<uint32_t>(sizeof(T))}; }
+};
+template <typename T>
+__device__ __forceinline__ uint32_t smem_u32(SPtr<T> p) {
+    return p.a;
+}
+// the value, cut off from how it was computed (kept in a register instead of being recomputed)
+__device__ __forceinline__ uint32_t opaque_u32(uint32_t x) {
+    uint32_t y;
+    asm volatile("mov.u32 %0, %1;" : "=r"(y) : "r"(x));
+    return y;
+}
+
 // one lane of the (converged) warp; the compiler keeps the surrounding control flow warp-uniform
 // named barrier among n threads (whole warps) of the CTA; id 1..15 (0 is __syncthreads)
 __device__ __forceinline__ void named_bar_sync(int id, int n) {
@@ -38,7 +58,8 @@ __device__ __forceinline__ bool elect_one() {
 }
 
 // explicit shared-memory accesses (a pointer that went through a function argument is generic to the compiler)
-__device__ __forceinline__ void st_shared_v2(const void* p, float a, float b) {
+template <typename A>
+__device__ __forceinline__ void st_shared_v2(A p, float a, float b) {
     asm volatile("st.shared.v2.f32 [%0], {%1, %2};" ::"r"(smem_u32(p)), "f"(a), "f"(b) : "memory");
 }
 __device__ __forceinline__ void st_shared_v4(const void* p, uint32_t a, uint32_t b, uint32_t c, uint32_t d) {
@@ -46,12 +67,14 @@ __device__ __forceinline__ void st_shared_v4(const void* p, uint32_t a, uint32_t
 }
 // (volatile: the load stays where it is written -- a role reads its own copy of a value after its setmaxnreg instead
 // of inheriting one that the common prologue has spilled)
-__device__ __forceinline__ uint32_t ld_shared_u32(const void* p) {
+template <typename A>
+__device__ __forceinline__ uint32_t ld_shared_u32(A p) {
     uint32_t r;
     asm volatile("ld.shared.u32 %0, [%1];" : "=r"(r) : "r"(smem_u32(p)) : "memory");
     return r;
 }
-__device__ __forceinline__ float2 ld_shared_v2(const void* p) {
+template <typename A>
+__device__ __forceinline__ float2 ld_shared_v2(A p) {
     float2 r;
     asm volatile("ld.shared.v2.f32 {%0, %1}, [%2];" : "=f"(r.x), "=f"(r.y) : "r"(smem_u32(p)) : "memory");
     return r;
@@ -68,14 +91,17 @@ __device__ __forceinline__ void fence_mbar_init() {
 __device__ __forceinline__ void fence_proxy_async_smem() {
     asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
 }
-__device__ __forceinline__ void mbar_arrive_expect_tx(uint64_t* bar, uint32_t bytes) {
+template <typename B>
+__device__ __forceinline__ void mbar_arrive_expect_tx(B bar, uint32_t bytes) {
     asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(bar)), "r"(bytes)
                  : "memory");
 }
-__device__ __forceinline__ void mbar_arrive(uint64_t* bar) {
+template <typename B>
+__device__ __forceinline__ void mbar_arrive(B bar) {
     asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(smem_u32(bar)) : "memory");
 }
-__device__ __forceinline__ bool mbar_try_wait(uint64_t* bar, uint32_t parity) {
+template <typename B>
+__device__ __forceinline__ bool mbar_try_wait(B bar, uint32_t parity) {
     uint32_t ok;
     asm volatile(
         "{\n\t.reg .pred p;\n\t"
@@ -87,7 +113,8 @@ __device__ __forceinline__ bool mbar_try_wait(uint64_t* bar, uint32_t parity) {
     return ok != 0;
 }
 // non-blocking probe (try_wait may suspend the thread for a while before it reports "not yet")
-__device__ __forceinline__ bool mbar_test_wait(uint64_t* bar, uint32_t parity) {
+template <typename B>
+__device__ __forceinline__ bool mbar_test_wait(B bar, uint32_t parity) {
     uint32_t ok;
     asm volatile(
         "{\n\t.reg .pred p;\n\t"
@@ -103,7 +130,8 @@ __device__ __forceinline__ bool mbar_test_wait(uint64_t* bar, uint32_t parity) {
 // the stack and reload them at the join after EVERY wait -- a local-memory round trip on the path barrier -> TMEM
 // load of each block (measured on cfg3, see profiles/r2_prefill_cfg3.md).  -DFP8ATTN_DEBUG_MBAR brings the
 // message back for debugging.
-__device__ __forceinline__ void mbar_wait(uint64_t* bar, uint32_t parity) {
+template <typename B>
+__device__ __forceinline__ void mbar_wait(B bar, uint32_t parity) {
     if (mbar_try_wait(bar, parity)) return;
     const long long t0 = clock64();
     while (!mbar_try_wait(bar, parity)) {
@@ -122,7 +150,8 @@ __device__ __forceinline__ void mbar_wait(uint64_t* bar, uint32_t parity) {
 // issuing independent work, and mbar_probe_result() reads the predicate later.  test_wait, not try_wait: a
 // try_wait on a phase that is not complete yet suspends the warp, a probe must never block.
 #define FP8ATTN_DECL_PROBE_PRED() asm volatile(".reg .pred fp8attn_probe_p;")
-__device__ __forceinline__ void mbar_probe(uint64_t* bar, uint32_t parity) {
+template <typename B>
+__device__ __forceinline__ void mbar_probe(B bar, uint32_t parity) {
     asm volatile("mbarrier.test_wait.parity.shared::cta.b64 fp8attn_probe_p, [%0], %1;" ::"r"(smem_u32(bar)), "r"(parity)
                  : "memory");
 }
@@ -137,7 +166,8 @@ __device__ __forceinline__ void prefetch_tmap(const CUtensorMap* m) {
     asm volatile("prefetch.tensormap [%0];" ::"l"(reinterpret_cast<uint64_t>(m)) : "memory");
 }
 // 3-D tiled load global -> shared, completion counted in bytes on `bar`.
-__device__ __forceinline__ void tma_load_3d(void* smem_dst, const CUtensorMap* m, uint64_t* bar, int c0,
+template <typename D, typename B>
+__device__ __forceinline__ void tma_load_3d(D smem_dst, const CUtensorMap* m, B bar, int c0,
                                             int c1, int c2) {
     asm volatile(
         "cp.async.bulk.tensor.3d.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1, {%3, %4, %5}], [%2];"
@@ -194,7 +224,8 @@ __device__ __forceinline__ void tmem_wait_st() { asm volatile("tcgen05.wait::st.
 
 // All MMAs issued so far by this thread arrive (once) on `bar` when they complete.
 // Implies tcgen05.fence::before_thread_sync.
-__device__ __forceinline__ void tc_commit(uint64_t* bar) {
+template <typename B>
+__device__ __forceinline__ void tc_commit(B bar) {
     asm volatile("tcgen05.commit.cta_group::1.mbarrier::arrive::one.shared::cluster.b64 [%0];" ::"r"(smem_u32(bar))
                  : "memory");
 }
