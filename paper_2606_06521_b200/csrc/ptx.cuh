@@ -128,7 +128,7 @@ __device__ __forceinline__ bool mbar_test_wait(B bar, uint32_t parity) {
 // Wait for the phase with the given parity to complete.  Traps (instead of hanging) if the barrier never flips.
 // The trap path makes no call: a printf here (an ABI call) makes ptxas keep loop-invariant values of the caller on
 // the stack and reload them at the join after EVERY wait -- a local-memory round trip on the path barrier -> TMEM
-// load of each block (measured on cfg3, see profiles/r2_prefill_cfg3.md).  -DFP8ATTN_DEBUG_MBAR brings the
+// load of each block (measured on cfg3, see profiles/r2b_prefill_cfg3.md).  -DFP8ATTN_DEBUG_MBAR brings the
 // message back for debugging.
 template <typename B>
 __device__ __forceinline__ void mbar_wait(B bar, uint32_t parity) {
